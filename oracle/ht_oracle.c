@@ -1,0 +1,242 @@
+/*
+ * ht_oracle.c -- CPU ORACLE for the Hough-Transform track finder of Rinaldi et al.,
+ * "GPGPU for track finding in High Energy Physics" (arXiv:1507.03074; /root/reference/PAPER.md).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may call it.  It shares no code with the CUDA
+ * library (paper_1507_03074_b200/csrc): no headers, helpers, tables or constants.
+ *
+ * It is the plain definition, single-threaded, in the paper's order:
+ *   - fill  : PAPER.md:25 (section 2): for every hit, every circle x^2+y^2-2Ax-2By=0 through the hit
+ *             and the origin; "for each A, the corresponding B is evaluated";
+ *             the M_H(A,B,theta,phi) element is "incremented by one".
+ *   - peaks : "elements above a given threshold ... local maxima search";
+ *             PAPER.md:43 "compares one M_H element to its neighbours and, if the biggest, it is stored".
+ * Where the paper is silent the readings R1-R16 of /root/repo/SPEC.md apply (listed in DESIGN.md).
+ *
+ * Precision: the paper does not fix one.  Floating point here DECIDES INTEGERS (bin indices), so both
+ * sides take those decisions in the kernel's precision: IEEE binary32, one rounding per operation,
+ * no FMA contraction.  Build: gcc -O2 -std=c11 -ffp-contract=off -fno-fast-math (x86-64 => SSE2 scalar).
+ *
+ * Pins (tests/test_oracle_*.py, all independent of this file's arithmetic): circle equation in double
+ * for every vote (P1), noiseless 12-layer track => one cell with 12 (P2), vote conservation (P3),
+ * cell-centric brute force in double with atan2 binning on tiny binnings (P4), single-hit geometry (P5),
+ * mirror symmetry (P6), permutation/batching invariance (P7), hand-built peak matrices (P8),
+ * peak-set invariants (P9), table binning vs atan2 (P10), closed-form in-range fraction.
+ * Parity unpinned by the paper (definitions fixed by SPEC.md only): R2/R4 angle definition and
+ * ranges, R5 bin centre, R10 neighbourhood, R11 >= vs >, R12 tie rule.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+typedef struct {
+    int32_t n_theta, n_phi, n_a, n_b;
+    float a_min, a_max, b_min, b_max;
+    float theta_min, theta_max, phi_min, phi_max;
+} oracle_binning;
+
+typedef struct { uint32_t event, cell, count; } oracle_peak;
+
+#define ORACLE_PI 3.14159265358979323846
+
+static double cot_d(double t) { return cos(t) / sin(t); }
+
+/* SPEC.md section 1: "diamond" pseudo-angle of an edge, evaluated in double. */
+static double pseudo_d(double phi)
+{
+    double c = cos(phi), s = sin(phi);
+    double m = fabs(c) + fabs(s);
+    return (s >= 0.0) ? 1.0 - c / m : 3.0 + c / m;
+}
+
+static int binning_ok(const oracle_binning *g)
+{
+    if (!g) return 0;
+    if (g->n_theta < 1 || g->n_phi < 1 || g->n_a < 1 || g->n_b < 1) return 0;
+    if (!(g->a_min < g->a_max) || !(g->b_min < g->b_max)) return 0;
+    if (!(g->theta_min < g->theta_max) || !(g->phi_min < g->phi_max)) return 0;
+    if (!isfinite(g->a_min) || !isfinite(g->a_max) || !isfinite(g->b_min) || !isfinite(g->b_max)) return 0;
+    return 1;
+}
+
+/*
+ * SPEC.md section 1.  two_a[NA]; t_theta[Ntheta+1] (index 0 and Ntheta = outer bounds);
+ * p_phi[Nphi+1] (same); d_ab[2] = {dA, dB}.
+ */
+int oracle_tables(const oracle_binning *g, float *two_a, float *t_theta, float *p_phi, float *d_ab)
+{
+    if (!binning_ok(g)) return -1;
+    float dA = (g->a_max - g->a_min) / (float)g->n_a;
+    float dB = (g->b_max - g->b_min) / (float)g->n_b;
+    d_ab[0] = dA;
+    d_ab[1] = dB;
+    for (int i = 0; i < g->n_a; ++i) {
+        float fi = (float)i + 0.5f;
+        float ac = g->a_min + fi * dA;          /* bin centre, R5 */
+        two_a[i] = 2.0f * ac;
+    }
+    int th_full_hi = g->theta_max >= (float)ORACLE_PI;
+    int ph_full_hi = g->phi_max >= (float)(2.0 * ORACLE_PI);
+    double thlo = (double)g->theta_min, thhi = th_full_hi ? ORACLE_PI : (double)g->theta_max;
+    double phlo = (double)g->phi_min, phhi = ph_full_hi ? 2.0 * ORACLE_PI : (double)g->phi_max;
+    t_theta[0] = (g->theta_min <= 0.0f) ? INFINITY : (float)cot_d(thlo);
+    for (int k = 1; k < g->n_theta; ++k) {
+        double th = thlo + ((thhi - thlo) * (double)k) / (double)g->n_theta;
+        t_theta[k] = (float)cot_d(th);
+    }
+    t_theta[g->n_theta] = th_full_hi ? -INFINITY : (float)cot_d(thhi);
+    p_phi[0] = (g->phi_min <= 0.0f) ? 0.0f : (float)pseudo_d(phlo);
+    for (int k = 1; k < g->n_phi; ++k) {
+        double ph = phlo + ((phhi - phlo) * (double)k) / (double)g->n_phi;
+        p_phi[k] = (float)pseudo_d(ph);
+    }
+    p_phi[g->n_phi] = ph_full_hi ? 4.0f : (float)pseudo_d(phhi);
+    return 0;
+}
+
+typedef struct {
+    const oracle_binning *g;
+    float *two_a, *t_theta, *p_phi;
+    float dA, dB;
+} tables;
+
+static int tables_make(tables *t, const oracle_binning *g)
+{
+    memset(t, 0, sizeof *t);
+    t->g = g;
+    t->two_a = (float *)malloc(sizeof(float) * (size_t)g->n_a);
+    t->t_theta = (float *)malloc(sizeof(float) * (size_t)(g->n_theta + 1));
+    t->p_phi = (float *)malloc(sizeof(float) * (size_t)(g->n_phi + 1));
+    float d[2];
+    if (!t->two_a || !t->t_theta || !t->p_phi || oracle_tables(g, t->two_a, t->t_theta, t->p_phi, d) != 0) {
+        free(t->two_a); free(t->t_theta); free(t->p_phi);
+        return -1;
+    }
+    t->dA = d[0];
+    t->dB = d[1];
+    return 0;
+}
+
+static void tables_free(tables *t) { free(t->two_a); free(t->t_theta); free(t->p_phi); }
+
+/* SPEC.md section 2, first half: the (theta,phi) plane of a hit, or -1 (R2, R3, R4, R8). */
+static int32_t hit_plane(const tables *t, float x, float y, float z)
+{
+    const oracle_binning *g = t->g;
+    float r2 = x * x + y * y;
+    float q = z / sqrtf(r2);
+    if (!(q <= t->t_theta[0] && q > t->t_theta[g->n_theta])) return -1;
+    int it = 0;
+    for (int k = 1; k < g->n_theta; ++k)
+        if (q <= t->t_theta[k]) ++it;
+    float d = fabsf(x) + fabsf(y);
+    float u = x / d;
+    float p = (y >= 0.0f) ? (1.0f - u) : (3.0f + u);
+    if (!(p >= t->p_phi[0] && p < t->p_phi[g->n_phi])) return -1;
+    int ip = 0;
+    for (int k = 1; k < g->n_phi; ++k)
+        if (p >= t->p_phi[k]) ++ip;
+    return (int32_t)(it * g->n_phi + ip);
+}
+
+/* SPEC.md section 2, second half: the B bin voted by hit (x,y) in A row i, or -1 (R5, R6, R7, R8). */
+static int32_t vote_bin(const tables *t, float x, float y, int i)
+{
+    float r2 = x * x + y * y;
+    float den = 2.0f * y;
+    float prod = t->two_a[i] * x;
+    float num = r2 - prod;
+    float B = num / den;                         /* B = (x^2+y^2-2Ax)/(2y) */
+    float s = B - t->g->b_min;
+    float tt = s / t->dB;
+    if (tt >= 0.0f && tt < (float)t->g->n_b) return (int32_t)tt;
+    return -1;
+}
+
+/*
+ * Fill the vote matrix of ONE event.  M (cells uint32) is zeroed here.  Returns the number of votes
+ * cast (-1 on bad arguments).  PAPER.md:25, 39-43.
+ */
+int64_t oracle_fill(const oracle_binning *g, const float *x, const float *y, const float *z, int64_t n_hits,
+                    uint32_t *M)
+{
+    tables t;
+    if (!binning_ok(g) || n_hits < 0 || !M || tables_make(&t, g) != 0) return -1;
+    size_t cells = (size_t)g->n_theta * (size_t)g->n_phi * (size_t)g->n_a * (size_t)g->n_b;
+    memset(M, 0, cells * sizeof(uint32_t));
+    int64_t votes = 0;
+    for (int64_t h = 0; h < n_hits; ++h) {
+        int32_t plane = hit_plane(&t, x[h], y[h], z[h]);
+        if (plane < 0) continue;
+        for (int i = 0; i < g->n_a; ++i) {
+            int32_t b = vote_bin(&t, x[h], y[h], i);
+            if (b < 0) continue;
+            size_t cell = ((size_t)plane * (size_t)g->n_a + (size_t)i) * (size_t)g->n_b + (size_t)b;
+            M[cell] += 1u;                       /* "incremented by one" */
+            ++votes;
+        }
+    }
+    tables_free(&t);
+    return votes;
+}
+
+/*
+ * The same decisions as oracle_fill, without the matrix: plane[h] (or -1) and bins[h*NA + i] (or -1).
+ * Exists so that tests can check every single vote against the circle equation (pin P1) and count
+ * votes without a matrix (pin P3).
+ */
+int oracle_votes(const oracle_binning *g, const float *x, const float *y, const float *z, int64_t n_hits,
+                 int32_t *plane, int32_t *bins)
+{
+    tables t;
+    if (!binning_ok(g) || n_hits < 0 || tables_make(&t, g) != 0) return -1;
+    for (int64_t h = 0; h < n_hits; ++h) {
+        plane[h] = hit_plane(&t, x[h], y[h], z[h]);
+        for (int i = 0; i < g->n_a; ++i)
+            bins[h * (int64_t)g->n_a + i] = (plane[h] < 0) ? -1 : vote_bin(&t, x[h], y[h], i);
+    }
+    tables_free(&t);
+    return 0;
+}
+
+/*
+ * Peak search over ONE event's matrix (SPEC.md section 3).  Emits peaks in increasing
+ * cell order; writes at most `capacity`; returns the number found (-1 on bad arguments).
+ */
+int64_t oracle_peaks(const oracle_binning *g, const uint32_t *M, uint32_t threshold, uint32_t event,
+                     oracle_peak *out, int64_t capacity)
+{
+    if (!binning_ok(g) || !M || threshold < 1u || capacity < 0) return -1;
+    const int64_t NA = g->n_a, NB = g->n_b, P = (int64_t)g->n_theta * g->n_phi;
+    int64_t found = 0;
+    for (int64_t p = 0; p < P; ++p) {
+        const uint32_t *plane = M + (size_t)p * (size_t)NA * (size_t)NB;
+        for (int64_t a = 0; a < NA; ++a) {
+            for (int64_t b = 0; b < NB; ++b) {
+                uint32_t c = plane[a * NB + b];
+                if (c < threshold) continue;                     /* R11 */
+                int is_peak = 1;
+                for (int da = -1; da <= 1 && is_peak; ++da) {
+                    for (int db = -1; db <= 1; ++db) {
+                        if (da == 0 && db == 0) continue;
+                        int64_t a2 = a + da, b2 = b + db;
+                        if (a2 < 0 || a2 >= NA || b2 < 0 || b2 >= NB) continue;   /* R10 */
+                        uint32_t nb = plane[a2 * NB + b2];
+                        int earlier = (da < 0) || (da == 0 && db < 0);
+                        if (earlier ? (nb >= c) : (nb > c)) { is_peak = 0; break; }  /* R12 */
+                    }
+                }
+                if (!is_peak) continue;
+                if (found < capacity) {
+                    out[found].event = event;
+                    out[found].cell = (uint32_t)((p * NA + a) * NB + b);
+                    out[found].count = c;
+                }
+                ++found;
+            }
+        }
+    }
+    return found;
+}

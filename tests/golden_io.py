@@ -1,0 +1,68 @@
+"""Reader of tests/golden/peak_cases.txt (format described in the file's header)."""
+from __future__ import annotations
+
+import os
+
+import numpy as np
+
+HERE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def read_peak_cases(path: str | None = None):
+    path = path or os.path.join(HERE, "peak_cases.txt")
+    cases, cur, plane_rows, plane_idx = [], None, None, None
+
+    def flush_plane():
+        nonlocal plane_rows, plane_idx
+        if plane_idx is not None:
+            arr = np.array(plane_rows, dtype=np.uint32)
+            assert arr.shape == (cur["dims"][2], cur["dims"][3]), (cur["name"], arr.shape)
+            cur["m"][plane_idx] = arr
+        plane_rows, plane_idx = None, None
+
+    with open(path) as f:
+        for raw in f:
+            line = raw.strip()
+            if not line or line.startswith("#"):
+                continue
+            tok = line.split()
+            if tok[0] == "case":
+                cur = {"name": tok[1]}
+            elif tok[0] == "dims":
+                cur["dims"] = tuple(int(t) for t in tok[1:5])
+                nt, nphi, na, nb = cur["dims"]
+                cur["m"] = np.zeros((nt * nphi, na, nb), np.uint32)
+            elif tok[0] == "T":
+                cur["T"] = int(tok[1])
+            elif tok[0] == "plane":
+                flush_plane()
+                plane_idx, plane_rows = int(tok[1]), []
+            elif tok[0] == "peaks":
+                flush_plane()
+                nt, nphi, na, nb = cur["dims"]
+                cells = []
+                for t in tok[1:]:
+                    p, a, b = (int(v) for v in t.split(":"))
+                    cells.append((p * na + a) * nb + b)
+                cur["peaks"] = sorted(cells)
+            elif tok[0] == "end":
+                nt, nphi, na, nb = cur["dims"]
+                cur["m"] = cur["m"].reshape(nt, nphi, na, nb)
+                cases.append(cur)
+                cur = None
+            else:
+                plane_rows.append([int(t) for t in tok])
+    return cases
+
+
+def read_paper_shapes(path: str | None = None) -> dict:
+    path = path or os.path.join(HERE, "paper_shapes.txt")
+    out = {}
+    with open(path) as f:
+        for raw in f:
+            line = raw.strip()
+            if not line or line.startswith("#"):
+                continue
+            k, *v = line.split()
+            out[k] = [float(t) if "." in t else int(t) for t in v]
+    return out
