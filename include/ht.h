@@ -1,0 +1,148 @@
+/*
+ * ht.h -- C ABI of libht: Hough-Transform track finding hot path on NVIDIA B200 (sm_100a).
+ *
+ * Method: Rinaldi et al., "GPGPU for track finding in High Energy Physics" (arXiv:1507.03074;
+ * /root/reference/PAPER.md).  Two steps (section 2):
+ *   1. fill : for each hit (x,y,z), all circles x^2+y^2-2Ax-2By=0 through the hit and the origin;
+ *             "for each A, the corresponding B is evaluated" and the element
+ *             M_H(A,B,theta,phi) of the vote matrix is "incremented by one";
+ *   2. peaks: "all the M_H elements above a given threshold would correspond to real tracks ... the
+ *             second step is a local maxima search"; "each thread compares one element
+ *             to its neighbours and, if the biggest, it is stored".
+ * Everything the paper leaves open (angle binning, bin centre, range ends, neighbourhood, ties) is
+ * fixed by /root/repo/SPEC.md (readings R1-R16); this library implements exactly that text.
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers (on cfg.device), h_* are HOST pointers.  The caller owns every
+ *     buffer it passes; the library owns only the ht_ctx (host struct + small device workspace: tables,
+ *     bucketed hits, per-(event,plane) offsets, counters; and, if cfg.host_slots > 0, staging buffers
+ *     and host_slots vote matrices for ht_run_host).
+ *   - Layout of a vote matrix (R15): uint32 M[event][itheta][iphi][ia][ib], ib fastest;
+ *     cell = ((itheta*Nphi + iphi)*NA + ia)*NB + ib  (< 2^32 required).  d_mh must be 16-byte aligned.
+ *   - ht_fill / ht_fill_naive / ht_peaks only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
+ *     void*, e.g. torch.cuda.Stream().cuda_stream; NULL = the legacy default stream).  No host
+ *     synchronisation, no allocation.  Results are valid once the caller has synchronised the stream.
+ *     Calls on one context must be stream-ordered with respect to each other (a context is not
+ *     thread-safe and keeps per-call scratch); separate contexts are independent.
+ *   - Every function returns HT_OK (0) or a negative ht_status; nothing aborts or throws.
+ *     ht_strerror gives text; for HT_ERR_CUDA the text of the last CUDA error seen by this thread.
+ */
+#ifndef HT_H_
+#define HT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(_WIN32)
+#define HT_API
+#else
+#define HT_API __attribute__((visibility("default")))
+#endif
+
+typedef enum ht_status {
+    HT_OK = 0,
+    HT_ERR_INVALID_ARG = -1, /* null pointer, non-positive bins, min >= max, non-finite range, n_events > max_events,
+                                n_hits_total > max_hits, threshold == 0, cells >= 2^32 */
+    HT_ERR_UNSUPPORTED = -2, /* binning does not fit the slab kernel (see ht_fill) -- use ht_fill_naive */
+    HT_ERR_CUDA = -3,        /* a CUDA runtime call or a launch failed */
+    HT_ERR_NOMEM = -4        /* host or device allocation failed */
+} ht_status;
+
+typedef struct ht_ctx ht_ctx; /* opaque; created by ht_create, freed by ht_destroy */
+
+/* Binning of the Hough space and capacities.  Ranges are half-open [min,max); angles in radians, lengths in mm.
+ * "binned in 4 x 16 x 1024 x 1024 along the corresponding A, B, theta, phi" (reading R1:
+ * n_theta=4, n_phi=16, n_a=n_b=1024). */
+typedef struct ht_config {
+    int32_t n_theta, n_phi, n_a, n_b;  /* bins, all >= 1 */
+    float a_min, a_max, b_min, b_max;  /* finite, min < max */
+    float theta_min, theta_max;        /* 0 <= min < max <= pi   (max >= (float)pi means exactly pi)   */
+    float phi_min, phi_max;            /* 0 <= min < max <= 2pi  (max >= (float)(2pi) means exactly 2pi) */
+    int32_t max_events;                /* largest n_events of one ht_fill / ht_peaks call, >= 1 */
+    int32_t max_hits;                  /* largest n_hits_total of one ht_fill call, >= 1 */
+    int32_t device;                    /* CUDA ordinal */
+    int32_t host_slots;                /* >= 0: vote matrices owned by the context for ht_run_host (0: that call is unavailable) */
+    uint32_t host_peak_capacity;       /* peak-list capacity of the context's staging buffer for ht_run_host */
+} ht_config;
+
+typedef struct ht_peak {
+    uint32_t event; /* index of the event inside the call's batch */
+    uint32_t cell;  /* linear cell index inside that event's matrix */
+    uint32_t count; /* M_H value of the cell */
+} ht_peak;
+
+/* Sizes implied by a configuration: bytes of one event's matrix, and device bytes ht_create will allocate. */
+HT_API int ht_query_sizes(const ht_config *cfg, size_t *mh_bytes_per_event, size_t *ctx_device_bytes);
+
+/* Host-only: the tables the library builds and uploads (SPEC.md section 1), for bit-for-bit comparison in tests.
+ * two_a[n_a], t_theta[n_theta+1], p_phi[n_phi+1], d_ab[2] = {dA, dB}.  Needs no GPU. */
+HT_API int ht_tables_host(const ht_config *cfg, float *two_a, float *t_theta, float *p_phi, float *d_ab);
+
+/* Validate cfg, build and upload tables, allocate the workspace on cfg.device.  *out is set only on HT_OK. */
+HT_API int ht_create(const ht_config *cfg, ht_ctx **out);
+
+/*
+ * Fill the vote matrices of a batch of events (SPEC.md section 2).
+ *   d_x, d_y, d_z     device, float32 SoA, n_hits_total entries (mm); hits of event e are
+ *                     [d_event_offsets[e], d_event_offsets[e+1])
+ *   d_event_offsets   device, int32, n_events+1 entries, ascending, first 0, last n_hits_total
+ *   n_events, n_hits_total  host copies of the sizes (grid sizing); n_events may be 0 (no-op)
+ *   d_mh              device, n_events * cells uint32, FULLY OVERWRITTEN: every cell is stored exactly once
+ *                     (zero or its count); it need not be cleared beforehand.
+ * Kernels: classify+bucket hits by (event, plane); then each CTA builds (plane, A-tile) slabs as private
+ * shared-memory histograms and writes them with bulk (TMA) stores: no global atomics, no memset pass.
+ * HT_ERR_UNSUPPORTED if n_b % 4 != 0, one A row (n_b*4 bytes) exceeds the slab budget, or planes > 8192.
+ */
+HT_API int ht_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z,
+                   const int32_t *d_event_offsets, int32_t n_events, int32_t n_hits_total, uint32_t *d_mh,
+                   void *cuda_stream);
+
+/* The paper's own design (cudaMemset, one block per hit, threads over A, global atomicAdd),
+ * same arguments and result as ht_fill, any binning.  Kept as the prior-art comparison and for shapes ht_fill
+ * refuses. */
+HT_API int ht_fill_naive(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z,
+                         const int32_t *d_event_offsets, int32_t n_events, int32_t n_hits_total, uint32_t *d_mh,
+                         void *cuda_stream);
+
+/*
+ * Thresholded local-maxima search with compaction (SPEC.md section 3).
+ *   d_mh        device, n_events * cells uint32 (as written by ht_fill)
+ *   threshold   >= 1 (count >= threshold is "above threshold", R11)
+ *   d_out       device, room for `capacity` records; order unspecified (compare after sorting by (event, cell))
+ *   d_n_found   device, one uint32: the number of peaks found, which may exceed capacity (then only
+ *               `capacity` records were written; not an error)
+ */
+HT_API int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_t threshold, ht_peak *d_out,
+                    uint32_t capacity, uint32_t *d_n_found, void *cuda_stream);
+
+/*
+ * End-to-end call with HOST buffers (needs cfg.host_slots >= 1): copies the hits to the device, runs ht_fill and
+ * ht_peaks on the context's own matrices (events in groups of host_slots), copies the peak list and count back
+ * and synchronises.  h_out receives min(*h_n_found, capacity) records; capacity <= cfg.host_peak_capacity.
+ * h_mh_or_null: if not NULL, n_events * cells uint32 that also receive the matrices (testing; slow).
+ * Host buffers may be pageable or pinned (pinned makes the copies asynchronous DMA).
+ */
+HT_API int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_z,
+                       const int32_t *h_event_offsets, int32_t n_events, int32_t n_hits_total, uint32_t threshold,
+                       ht_peak *h_out, uint32_t capacity, uint32_t *h_n_found, uint32_t *h_mh_or_null);
+
+/* Number of kernels this context has launched so far (host-side counter; for bench.py's gpu_launches). */
+HT_API int64_t ht_kernel_launches(const ht_ctx *ctx);
+
+/* Launch geometry of the last ht_fill / ht_peaks (for DESIGN.md / bench reporting): out[0]=fill grid, out[1]=fill block,
+ * out[2]=fill dynamic smem bytes, out[3]=rows per slab, out[4]=peaks grid, out[5]=peaks block, out[6]=SM count, out[7]=0. */
+HT_API int ht_launch_info(const ht_ctx *ctx, int32_t out[8]);
+
+/* Free everything the context owns.  NULL is allowed. */
+HT_API void ht_destroy(ht_ctx *ctx);
+
+HT_API const char *ht_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HT_H_ */

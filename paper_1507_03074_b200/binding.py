@@ -1,0 +1,179 @@
+"""Thin ctypes binding of libht.so -- the same names as include/ht.h, argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind these calls; nothing here computes.  There is no CPU
+fallback: if the library is missing or does not load, importing a function from here raises.  PyTorch appears only
+as the owner of device memory and streams (``tensor.data_ptr()``, ``torch.cuda.Stream().cuda_stream``).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libht.so")
+
+HT_OK, HT_ERR_INVALID_ARG, HT_ERR_UNSUPPORTED, HT_ERR_CUDA, HT_ERR_NOMEM = 0, -1, -2, -3, -4
+
+PEAK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32)])   # == struct ht_peak
+
+EXPORTS = ("ht_query_sizes", "ht_tables_host", "ht_create", "ht_fill", "ht_fill_naive", "ht_peaks", "ht_run_host",
+           "ht_kernel_launches", "ht_launch_info", "ht_destroy", "ht_strerror")
+
+
+class ht_config(C.Structure):
+    _fields_ = [("n_theta", C.c_int32), ("n_phi", C.c_int32), ("n_a", C.c_int32), ("n_b", C.c_int32),
+                ("a_min", C.c_float), ("a_max", C.c_float), ("b_min", C.c_float), ("b_max", C.c_float),
+                ("theta_min", C.c_float), ("theta_max", C.c_float), ("phi_min", C.c_float), ("phi_max", C.c_float),
+                ("max_events", C.c_int32), ("max_hits", C.c_int32), ("device", C.c_int32),
+                ("host_slots", C.c_int32), ("host_peak_capacity", C.c_uint32)]
+
+    @classmethod
+    def from_binning(cls, b, *, max_events: int, max_hits: int, device: int = 0, host_slots: int = 0,
+                     host_peak_capacity: int = 0) -> "ht_config":
+        return cls(b.n_theta, b.n_phi, b.n_a, b.n_b, b.a_min, b.a_max, b.b_min, b.b_max, b.theta_min, b.theta_max,
+                   b.phi_min, b.phi_max, max_events, max_hits, device, host_slots, host_peak_capacity)
+
+    @property
+    def cells(self) -> int:
+        return self.n_theta * self.n_phi * self.n_a * self.n_b
+
+
+class HtError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {ht_strerror(status)} (status {status})")
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """Load libht.so (built in-tree by paper_1507_03074_b200/build.py).  Fails loudly: there is no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1507_03074_b200.build` "
+                          "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, u32 = C.c_void_p, C.c_int32, C.c_uint32
+    cfgp = C.POINTER(ht_config)
+    lib.ht_query_sizes.restype = C.c_int
+    lib.ht_query_sizes.argtypes = [cfgp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+    lib.ht_tables_host.restype = C.c_int
+    lib.ht_tables_host.argtypes = [cfgp, vp, vp, vp, vp]
+    lib.ht_create.restype = C.c_int
+    lib.ht_create.argtypes = [cfgp, C.POINTER(vp)]
+    for name in ("ht_fill", "ht_fill_naive"):
+        fn = getattr(lib, name)
+        fn.restype = C.c_int
+        fn.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, vp]
+    lib.ht_peaks.restype = C.c_int
+    lib.ht_peaks.argtypes = [vp, vp, i32, u32, vp, u32, vp, vp]
+    lib.ht_run_host.restype = C.c_int
+    lib.ht_run_host.argtypes = [vp, vp, vp, vp, vp, i32, i32, u32, vp, u32, vp, vp]
+    lib.ht_kernel_launches.restype = C.c_int64
+    lib.ht_kernel_launches.argtypes = [vp]
+    lib.ht_launch_info.restype = C.c_int
+    lib.ht_launch_info.argtypes = [vp, C.POINTER(i32 * 8)]
+    lib.ht_destroy.restype = None
+    lib.ht_destroy.argtypes = [vp]
+    lib.ht_strerror.restype = C.c_char_p
+    lib.ht_strerror.argtypes = [C.c_int]
+    _lib = lib
+    return lib
+
+
+def _ptr(a) -> int | None:
+    """Address of a torch tensor / numpy array / int / None (marshalling only)."""
+    if a is None:
+        return None
+    if isinstance(a, int):
+        return a
+    if isinstance(a, np.ndarray):
+        return a.ctypes.data
+    return a.data_ptr()          # torch.Tensor
+
+
+def _stream(s) -> int | None:
+    if s is None:
+        return None
+    if isinstance(s, int):
+        return s or None
+    return s.cuda_stream or None  # torch.cuda.Stream
+
+
+def _check(status: int, where: str) -> None:
+    if status != HT_OK:
+        raise HtError(status, where)
+
+
+def ht_strerror(status: int) -> str:
+    return load().ht_strerror(status).decode()
+
+
+def ht_query_sizes(cfg: ht_config) -> tuple[int, int]:
+    """(bytes of one event's matrix, device bytes ht_create allocates)."""
+    a, b = C.c_size_t(), C.c_size_t()
+    _check(load().ht_query_sizes(C.byref(cfg), C.byref(a), C.byref(b)), "ht_query_sizes")
+    return a.value, b.value
+
+
+def ht_tables_host(cfg: ht_config):
+    """(two_a, t_theta, p_phi, dA, dB): the tables the library uploads (host only, needs no GPU)."""
+    two_a = np.empty(cfg.n_a, np.float32)
+    tth = np.empty(cfg.n_theta + 1, np.float32)
+    pph = np.empty(cfg.n_phi + 1, np.float32)
+    d = np.empty(2, np.float32)
+    _check(load().ht_tables_host(C.byref(cfg), _ptr(two_a), _ptr(tth), _ptr(pph), _ptr(d)), "ht_tables_host")
+    return two_a, tth, pph, np.float32(d[0]), np.float32(d[1])
+
+
+def ht_create(cfg: ht_config) -> int:
+    """Returns the opaque context handle (an address)."""
+    out = C.c_void_p()
+    _check(load().ht_create(C.byref(cfg), C.byref(out)), "ht_create")
+    return out.value
+
+
+def ht_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events: int, n_hits_total: int, d_mh, stream=None) -> None:
+    _check(load().ht_fill(ctx, _ptr(d_x), _ptr(d_y), _ptr(d_z), _ptr(d_event_offsets), n_events, n_hits_total,
+                          _ptr(d_mh), _stream(stream)), "ht_fill")
+
+
+def ht_fill_naive(ctx, d_x, d_y, d_z, d_event_offsets, n_events: int, n_hits_total: int, d_mh, stream=None) -> None:
+    _check(load().ht_fill_naive(ctx, _ptr(d_x), _ptr(d_y), _ptr(d_z), _ptr(d_event_offsets), n_events, n_hits_total,
+                                _ptr(d_mh), _stream(stream)), "ht_fill_naive")
+
+
+def ht_peaks(ctx, d_mh, n_events: int, threshold: int, d_out, capacity: int, d_n_found, stream=None) -> None:
+    _check(load().ht_peaks(ctx, _ptr(d_mh), n_events, threshold, _ptr(d_out), capacity, _ptr(d_n_found),
+                           _stream(stream)), "ht_peaks")
+
+
+def ht_run_host(ctx, h_x, h_y, h_z, h_event_offsets, n_events: int, n_hits_total: int, threshold: int, h_out,
+                capacity: int, h_mh=None) -> int:
+    """End-to-end call on HOST buffers (numpy arrays or pinned torch CPU tensors).  Returns the number of peaks found;
+    ``h_out`` (PEAK_DTYPE array or 3-column uint32 tensor) receives min(found, capacity) records."""
+    n = C.c_uint32(0)
+    _check(load().ht_run_host(ctx, _ptr(h_x), _ptr(h_y), _ptr(h_z), _ptr(h_event_offsets), n_events, n_hits_total,
+                              threshold, _ptr(h_out), capacity, C.addressof(n), _ptr(h_mh)), "ht_run_host")
+    return n.value
+
+
+def ht_kernel_launches(ctx) -> int:
+    return int(load().ht_kernel_launches(ctx))
+
+
+def ht_launch_info(ctx) -> dict:
+    arr = (C.c_int32 * 8)()
+    _check(load().ht_launch_info(ctx, C.byref(arr)), "ht_launch_info")
+    keys = ("fill_grid", "fill_block", "fill_smem_bytes", "rows_per_slab", "peaks_grid", "peaks_block", "sm_count")
+    return dict(zip(keys, list(arr)[:7]))
+
+
+def ht_destroy(ctx) -> None:
+    if ctx:
+        load().ht_destroy(ctx)

@@ -1,0 +1,490 @@
+// ht_api.cu -- C ABI of libht (include/ht.h): argument validation, table construction (SPEC.md section 1),
+// workspace management and kernel launches.  No torch types, no exceptions across the boundary.
+#include "../../include/ht.h"
+#include "ht_device.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace {
+
+thread_local char g_cuda_err[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    std::snprintf(g_cuda_err, sizeof g_cuda_err, "CUDA error in %s: %s", what, cudaGetErrorString(e));
+    return HT_ERR_CUDA;
+}
+
+#define HT_CUDA(call)                                        \
+    do {                                                     \
+        cudaError_t e__ = (call);                            \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+
+constexpr double kPi = 3.14159265358979323846;
+
+int env_int(const char *name, int dflt)
+{
+    const char *s = std::getenv(name);
+    if (!s || !*s) return dflt;
+    return std::atoi(s);
+}
+
+bool config_ok(const ht_config *c)
+{
+    if (!c) return false;
+    if (c->n_theta < 1 || c->n_phi < 1 || c->n_a < 1 || c->n_b < 1) return false;
+    const float r[8] = {c->a_min, c->a_max, c->b_min, c->b_max, c->theta_min, c->theta_max, c->phi_min, c->phi_max};
+    for (float v : r)
+        if (!std::isfinite(v)) return false;
+    if (!(c->a_min < c->a_max) || !(c->b_min < c->b_max)) return false;
+    if (!(c->theta_min < c->theta_max) || !(c->phi_min < c->phi_max)) return false;
+    if (c->theta_min < 0.0f || c->phi_min < 0.0f) return false;
+    if (c->theta_max > (float)kPi || c->phi_max > (float)(2.0 * kPi)) return false;
+    const unsigned long long cells =
+        (unsigned long long)c->n_theta * (unsigned long long)c->n_phi * (unsigned long long)c->n_a * (unsigned long long)c->n_b;
+    if (cells >= (1ull << 32)) return false;          // ht_peak.cell is uint32
+    if ((long long)c->n_theta * (long long)c->n_phi > (1ll << 30)) return false;
+    return true;
+}
+
+double cot(double t) { return std::cos(t) / std::sin(t); }
+
+// "diamond" pseudo-angle of an edge, in double (SPEC.md section 1)
+double pseudo_angle(double phi)
+{
+    const double c = std::cos(phi), s = std::sin(phi);
+    const double m = std::fabs(c) + std::fabs(s);
+    return (s >= 0.0) ? 1.0 - c / m : 3.0 + c / m;
+}
+
+void build_tables(const ht_config *c, float *two_a, float *tth, float *pph, float *d_ab)
+{
+    // volatile: one IEEE binary32 rounding per operation, whatever the host compiler's contraction setting
+    volatile float dA = (c->a_max - c->a_min) / (float)c->n_a;
+    volatile float dB = (c->b_max - c->b_min) / (float)c->n_b;
+    d_ab[0] = dA;
+    d_ab[1] = dB;
+    if (two_a) {
+        for (int i = 0; i < c->n_a; ++i) {
+            volatile float fi = (float)i + 0.5f;
+            volatile float prod = fi * dA;
+            volatile float ac = c->a_min + prod;
+            two_a[i] = 2.0f * ac;
+        }
+    }
+    const bool th_full = c->theta_max >= (float)kPi;
+    const bool ph_full = c->phi_max >= (float)(2.0 * kPi);
+    const double thlo = (double)c->theta_min, thhi = th_full ? kPi : (double)c->theta_max;
+    const double phlo = (double)c->phi_min, phhi = ph_full ? 2.0 * kPi : (double)c->phi_max;
+    tth[0] = (c->theta_min <= 0.0f) ? INFINITY : (float)cot(thlo);
+    for (int k = 1; k < c->n_theta; ++k) tth[k] = (float)cot(thlo + ((thhi - thlo) * (double)k) / (double)c->n_theta);
+    tth[c->n_theta] = th_full ? -INFINITY : (float)cot(thhi);
+    pph[0] = (c->phi_min <= 0.0f) ? 0.0f : (float)pseudo_angle(phlo);
+    for (int k = 1; k < c->n_phi; ++k) pph[k] = (float)pseudo_angle(phlo + ((phhi - phlo) * (double)k) / (double)c->n_phi);
+    pph[c->n_phi] = ph_full ? 4.0f : (float)pseudo_angle(phhi);
+}
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace
+
+struct ht_ctx {
+    ht_config cfg;
+    ht::Geom geom;
+    int sm_count = 0;
+    int max_smem_optin = 0;
+    // device workspace
+    float *d_tth = nullptr, *d_pph = nullptr;
+    ht::HitRec *d_rec = nullptr;
+    int32_t *d_plane_off = nullptr;
+    uint32_t *d_counters = nullptr;
+    // slab-fill launch geometry
+    bool slab_ok = false;
+    int rows_per_slab = 0, tiles_per_plane = 0, fill_threads = 0, fill_nbuf = 0, fill_ctas_per_sm = 0;
+    size_t slab_bytes = 0, fill_smem = 0, classify_smem = 0;
+    int peaks_ctas_per_sm = 0;
+    // host path (ht_run_host)
+    float *d_hx = nullptr, *d_hy = nullptr, *d_hz = nullptr;
+    int32_t *d_hoff = nullptr;
+    uint32_t *d_hmh = nullptr;
+    unsigned char *d_hres = nullptr;   // [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
+    unsigned char *h_res = nullptr;    // pinned mirror of d_hres
+    cudaStream_t host_stream = nullptr;
+    int64_t launches = 0;
+    int32_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+};
+
+namespace {
+
+constexpr size_t kResHeader = 16;
+
+struct WorkspaceSizes {
+    size_t rec, plane_off, tables, counters, host_hits, host_off, host_mh, host_res, total;
+};
+
+WorkspaceSizes workspace_sizes(const ht_config *c)
+{
+    WorkspaceSizes w{};
+    const size_t planes = (size_t)c->n_theta * (size_t)c->n_phi;
+    const size_t cells = planes * (size_t)c->n_a * (size_t)c->n_b;
+    w.rec = align_up(sizeof(ht::HitRec) * (size_t)c->max_hits, 256);
+    w.plane_off = align_up(sizeof(int32_t) * (size_t)c->max_events * (planes + 1), 256);
+    w.tables = align_up(sizeof(float) * (size_t)(c->n_theta + 1 + c->n_phi + 1), 256);
+    w.counters = 256;
+    if (c->host_slots > 0) {
+        w.host_hits = 3 * align_up(sizeof(float) * (size_t)c->max_hits, 256);
+        w.host_off = align_up(sizeof(int32_t) * ((size_t)c->max_events + 1), 256);
+        w.host_mh = align_up(cells * sizeof(uint32_t) * (size_t)c->host_slots, 256);
+        w.host_res = align_up(kResHeader + sizeof(ht_peak) * (size_t)c->host_peak_capacity, 256);
+    }
+    w.total = w.rec + w.plane_off + w.tables + w.counters + w.host_hits + w.host_off + w.host_mh + w.host_res;
+    return w;
+}
+
+// Slab geometry: rows per slab so that NBUF slabs of rows*NB*4 bytes fit `ctas_per_sm` CTAs into shared memory.
+void plan_fill(ht_ctx *ctx)
+{
+    const ht_config &c = ctx->cfg;
+    ctx->slab_ok = false;
+    const size_t row_bytes = (size_t)c.n_b * 4u;
+    const int slab_kb = env_int("HT_FILL_SLAB_KB", 48);
+    const int nbuf = env_int("HT_FILL_NBUF", 2);
+    const int threads = env_int("HT_FILL_THREADS", 512);
+    const int ctas = env_int("HT_FILL_CTAS_PER_SM", 2);
+    if (nbuf != 1 && nbuf != 2) return;
+    if (threads < 32 || threads > 1024 || (threads & 31)) return;
+    if (c.n_b % 4 != 0) return;
+    if ((long long)c.n_theta * c.n_phi > 8192) return;
+    const size_t budget = (size_t)slab_kb * 1024u;
+    if (row_bytes > budget || (size_t)nbuf * row_bytes > (size_t)ctx->max_smem_optin) return;
+    int rows = (int)(budget / row_bytes);
+    if (rows > c.n_a) rows = c.n_a;
+    while (rows > 1 && (size_t)nbuf * (size_t)rows * row_bytes > (size_t)ctx->max_smem_optin) --rows;
+    ctx->rows_per_slab = rows;
+    ctx->tiles_per_plane = (c.n_a + rows - 1) / rows;
+    ctx->slab_bytes = (size_t)rows * row_bytes;
+    ctx->fill_nbuf = nbuf;
+    ctx->fill_threads = threads;
+    ctx->fill_ctas_per_sm = ctas < 1 ? 1 : ctas;
+    ctx->fill_smem = (size_t)nbuf * ctx->slab_bytes;
+    ctx->slab_ok = true;
+}
+
+int check_fill_args(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off,
+                    int32_t n_events, int32_t n_hits_total, uint32_t *d_mh)
+{
+    if (!ctx) return HT_ERR_INVALID_ARG;
+    if (n_events < 0 || n_hits_total < 0) return HT_ERR_INVALID_ARG;
+    if (n_events > ctx->cfg.max_events || n_hits_total > ctx->cfg.max_hits) return HT_ERR_INVALID_ARG;
+    if (n_events == 0) return HT_OK;
+    if (!d_off || !d_mh) return HT_ERR_INVALID_ARG;
+    if (n_hits_total > 0 && (!d_x || !d_y || !d_z)) return HT_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_mh) & 15u) != 0) return HT_ERR_INVALID_ARG;
+    return HT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ht_query_sizes(const ht_config *cfg, size_t *mh_bytes_per_event, size_t *ctx_device_bytes)
+{
+    if (!config_ok(cfg) || cfg->max_events < 1 || cfg->max_hits < 1 || cfg->host_slots < 0) return HT_ERR_INVALID_ARG;
+    const size_t cells = (size_t)cfg->n_theta * (size_t)cfg->n_phi * (size_t)cfg->n_a * (size_t)cfg->n_b;
+    if (mh_bytes_per_event) *mh_bytes_per_event = cells * sizeof(uint32_t);
+    if (ctx_device_bytes) *ctx_device_bytes = workspace_sizes(cfg).total;
+    return HT_OK;
+}
+
+int ht_tables_host(const ht_config *cfg, float *two_a, float *t_theta, float *p_phi, float *d_ab)
+{
+    if (!config_ok(cfg) || !t_theta || !p_phi || !d_ab) return HT_ERR_INVALID_ARG;
+    build_tables(cfg, two_a, t_theta, p_phi, d_ab);
+    return HT_OK;
+}
+
+int ht_create(const ht_config *cfg, ht_ctx **out)
+{
+    if (!out) return HT_ERR_INVALID_ARG;
+    if (!config_ok(cfg) || cfg->max_events < 1 || cfg->max_hits < 1 || cfg->host_slots < 0) return HT_ERR_INVALID_ARG;
+    int ndev = 0;
+    HT_CUDA(cudaGetDeviceCount(&ndev));
+    if (cfg->device < 0 || cfg->device >= ndev) return HT_ERR_INVALID_ARG;
+    HT_CUDA(cudaSetDevice(cfg->device));
+
+    ht_ctx *ctx = new (std::nothrow) ht_ctx();
+    if (!ctx) return HT_ERR_NOMEM;
+    ctx->cfg = *cfg;
+    ht::Geom &g = ctx->geom;
+    g.n_theta = cfg->n_theta; g.n_phi = cfg->n_phi; g.n_a = cfg->n_a; g.n_b = cfg->n_b;
+    g.planes = cfg->n_theta * cfg->n_phi;
+    g.cells = (unsigned long long)g.planes * (unsigned long long)cfg->n_a * (unsigned long long)cfg->n_b;
+    std::vector<float> tth((size_t)cfg->n_theta + 1), pph((size_t)cfg->n_phi + 1);
+    float d_ab[2];
+    build_tables(cfg, nullptr, tth.data(), pph.data(), d_ab);
+    g.a_min = cfg->a_min; g.dA = d_ab[0]; g.b_min = cfg->b_min; g.dB = d_ab[1]; g.nb_f = (float)cfg->n_b;
+
+    cudaError_t e;
+    int rc = HT_OK;
+    auto fail = [&](int code) { ht_destroy(ctx); return code; };
+    if ((e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, cfg->device)) != cudaSuccess)
+        return fail(cuda_fail(e, "cudaDeviceGetAttribute(SM count)"));
+    if ((e = cudaDeviceGetAttribute(&ctx->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device)) != cudaSuccess)
+        return fail(cuda_fail(e, "cudaDeviceGetAttribute(smem optin)"));
+
+    const WorkspaceSizes w = workspace_sizes(cfg);
+    auto dmalloc = [&](void **p, size_t bytes, const char *what) -> bool {
+        if (bytes == 0) { *p = nullptr; return true; }
+        cudaError_t err = cudaMalloc(p, bytes);
+        if (err != cudaSuccess) {
+            rc = (err == cudaErrorMemoryAllocation) ? HT_ERR_NOMEM : cuda_fail(err, what);
+            if (err == cudaErrorMemoryAllocation) cudaGetLastError();
+            return false;
+        }
+        return true;
+    };
+    if (!dmalloc((void **)&ctx->d_rec, w.rec, "cudaMalloc(rec)")) return fail(rc);
+    if (!dmalloc((void **)&ctx->d_plane_off, w.plane_off, "cudaMalloc(plane_off)")) return fail(rc);
+    if (!dmalloc((void **)&ctx->d_tth, w.tables, "cudaMalloc(tables)")) return fail(rc);
+    ctx->d_pph = ctx->d_tth + (cfg->n_theta + 1);
+    if (!dmalloc((void **)&ctx->d_counters, w.counters, "cudaMalloc(counters)")) return fail(rc);
+    if ((e = cudaMemcpy(ctx->d_tth, tth.data(), tth.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMemcpy(ctx->d_pph, pph.data(), pph.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMemset(ctx->d_counters, 0, w.counters)) != cudaSuccess)
+        return fail(cuda_fail(e, "table upload"));
+
+    if (cfg->host_slots > 0) {
+        const size_t hb = align_up(sizeof(float) * (size_t)cfg->max_hits, 256);
+        if (!dmalloc((void **)&ctx->d_hx, w.host_hits, "cudaMalloc(host hits)")) return fail(rc);
+        ctx->d_hy = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ctx->d_hx) + hb);
+        ctx->d_hz = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ctx->d_hx) + 2 * hb);
+        if (!dmalloc((void **)&ctx->d_hoff, w.host_off, "cudaMalloc(host offsets)")) return fail(rc);
+        if (!dmalloc((void **)&ctx->d_hmh, w.host_mh, "cudaMalloc(host matrices)")) return fail(rc);
+        if (!dmalloc((void **)&ctx->d_hres, w.host_res, "cudaMalloc(host result)")) return fail(rc);
+        if ((e = cudaMallocHost((void **)&ctx->h_res, w.host_res)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaMallocHost(result)"));
+        if ((e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaStreamCreate"));
+    }
+
+    plan_fill(ctx);
+    ctx->classify_smem = sizeof(float) * (size_t)(cfg->n_theta + cfg->n_phi + 2) + sizeof(int) * (2 * (size_t)g.planes + 32);
+    if (ctx->slab_ok) {
+        if (ctx->classify_smem > (size_t)ctx->max_smem_optin) ctx->slab_ok = false;
+    }
+    if (ctx->slab_ok) {
+        if ((e = cudaFuncSetAttribute(ht::classify_bucket_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)ctx->classify_smem)) != cudaSuccess ||
+            (e = cudaFuncSetAttribute(ht::fill_slab_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)ctx->fill_smem)) != cudaSuccess ||
+            (e = cudaFuncSetAttribute(ht::fill_slab_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)ctx->fill_smem)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaFuncSetAttribute"));
+    }
+    ctx->peaks_ctas_per_sm = env_int("HT_PEAKS_CTAS_PER_SM", 8);
+    if (ctx->peaks_ctas_per_sm < 1) ctx->peaks_ctas_per_sm = 1;
+    ctx->info[6] = ctx->sm_count;
+    *out = ctx;
+    return HT_OK;
+}
+
+int ht_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
+            int32_t n_events, int32_t n_hits_total, uint32_t *d_mh, void *cuda_stream)
+{
+    const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh);
+    if (rc != HT_OK || n_events == 0) return rc;
+    if (!ctx->slab_ok) return HT_ERR_UNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const ht::Geom &g = ctx->geom;
+
+    ht::classify_bucket_kernel<<<n_events, ht::kClassifyThreads, ctx->classify_smem, st>>>(
+        d_x, d_y, d_z, d_event_offsets, ctx->d_tth, ctx->d_pph, g, ctx->d_rec, ctx->d_plane_off);
+    HT_CUDA(cudaGetLastError());
+    ++ctx->launches;
+
+    const long long n_items = (long long)n_events * g.planes * ctx->tiles_per_plane;
+    long long grid = (long long)ctx->sm_count * ctx->fill_ctas_per_sm;
+    if (grid > n_items) grid = n_items;
+    const uint32_t slab_words = (uint32_t)(ctx->slab_bytes / 4u);
+    if (ctx->fill_nbuf == 2)
+        ht::fill_slab_kernel<2><<<(unsigned)grid, ctx->fill_threads, ctx->fill_smem, st>>>(
+            ctx->d_rec, ctx->d_plane_off, g, ctx->rows_per_slab, ctx->tiles_per_plane, n_items, slab_words, d_mh);
+    else
+        ht::fill_slab_kernel<1><<<(unsigned)grid, ctx->fill_threads, ctx->fill_smem, st>>>(
+            ctx->d_rec, ctx->d_plane_off, g, ctx->rows_per_slab, ctx->tiles_per_plane, n_items, slab_words, d_mh);
+    HT_CUDA(cudaGetLastError());
+    ++ctx->launches;
+    ctx->info[0] = (int32_t)grid; ctx->info[1] = ctx->fill_threads; ctx->info[2] = (int32_t)ctx->fill_smem;
+    ctx->info[3] = ctx->rows_per_slab;
+    return HT_OK;
+}
+
+int ht_fill_naive(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
+                  int32_t n_events, int32_t n_hits_total, uint32_t *d_mh, void *cuda_stream)
+{
+    const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh);
+    if (rc != HT_OK || n_events == 0) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const ht::Geom &g = ctx->geom;
+    HT_CUDA(cudaMemsetAsync(d_mh, 0, (size_t)n_events * (size_t)g.cells * sizeof(uint32_t), st));
+    if (n_hits_total > 0) {
+        const int threads = g.n_a >= 256 ? 256 : ((g.n_a + 31) / 32) * 32;
+        ht::fill_naive_kernel<<<n_hits_total, threads, 0, st>>>(d_x, d_y, d_z, d_event_offsets, n_events, ctx->d_tth,
+                                                                ctx->d_pph, g, d_mh);
+        HT_CUDA(cudaGetLastError());
+        ++ctx->launches;
+    }
+    return HT_OK;
+}
+
+int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_t threshold, ht_peak *d_out,
+             uint32_t capacity, uint32_t *d_n_found, void *cuda_stream)
+{
+    if (!ctx || n_events < 0 || n_events > ctx->cfg.max_events || threshold < 1u || !d_n_found) return HT_ERR_INVALID_ARG;
+    if (capacity > 0 && !d_out) return HT_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (n_events == 0) {
+        HT_CUDA(cudaMemsetAsync(d_n_found, 0, sizeof(uint32_t), st));
+        return HT_OK;
+    }
+    if (!d_mh) return HT_ERR_INVALID_ARG;
+    const ht::Geom &g = ctx->geom;
+    const unsigned long long total_cells = (unsigned long long)n_events * g.cells;
+    const bool vec4 = (g.n_b % 4 == 0) && ((reinterpret_cast<uintptr_t>(d_mh) & 15u) == 0);
+    const unsigned long long n_groups = vec4 ? total_cells / 4ull : total_cells;
+    const unsigned long long per_cta = (unsigned long long)ht::kPeaksThreads * ht::kPeaksUnroll;
+    unsigned long long grid = (n_groups + per_cta - 1ull) / per_cta;
+    const unsigned long long cap = (unsigned long long)ctx->sm_count * (unsigned long long)ctx->peaks_ctas_per_sm;
+    if (grid > cap) grid = cap;
+    if (grid < 1ull) grid = 1ull;
+    static_assert(sizeof(ht::PeakOut) == sizeof(ht_peak), "peak record layout");
+    ht::PeakOut *out = reinterpret_cast<ht::PeakOut *>(d_out);
+    if (vec4)
+        ht::peaks_kernel<4><<<(unsigned)grid, ht::kPeaksThreads, 0, st>>>(d_mh, n_groups, g, threshold, out, capacity,
+                                                                         ctx->d_counters, d_n_found);
+    else
+        ht::peaks_kernel<1><<<(unsigned)grid, ht::kPeaksThreads, 0, st>>>(d_mh, n_groups, g, threshold, out, capacity,
+                                                                         ctx->d_counters, d_n_found);
+    HT_CUDA(cudaGetLastError());
+    ++ctx->launches;
+    ctx->info[4] = (int32_t)grid; ctx->info[5] = ht::kPeaksThreads;
+    return HT_OK;
+}
+
+int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_z, const int32_t *h_event_offsets,
+                int32_t n_events, int32_t n_hits_total, uint32_t threshold, ht_peak *h_out, uint32_t capacity,
+                uint32_t *h_n_found, uint32_t *h_mh_or_null)
+{
+    if (!ctx || !h_n_found) return HT_ERR_INVALID_ARG;
+    if (ctx->cfg.host_slots < 1) return HT_ERR_UNSUPPORTED;
+    if (n_events < 0 || n_hits_total < 0 || n_events > ctx->cfg.max_events || n_hits_total > ctx->cfg.max_hits)
+        return HT_ERR_INVALID_ARG;
+    if (threshold < 1u || capacity > ctx->cfg.host_peak_capacity || (capacity > 0 && !h_out)) return HT_ERR_INVALID_ARG;
+    *h_n_found = 0u;
+    if (n_events == 0) return HT_OK;
+    if (!h_event_offsets || (n_hits_total > 0 && (!h_x || !h_y || !h_z))) return HT_ERR_INVALID_ARG;
+    if (h_event_offsets[0] != 0 || h_event_offsets[n_events] != n_hits_total) return HT_ERR_INVALID_ARG;
+    for (int e = 0; e < n_events; ++e)
+        if (h_event_offsets[e] > h_event_offsets[e + 1]) return HT_ERR_INVALID_ARG;
+
+    cudaStream_t st = ctx->host_stream;
+    const size_t cells = (size_t)ctx->geom.cells;
+    if (n_hits_total > 0) {
+        const size_t nb = sizeof(float) * (size_t)n_hits_total;
+        HT_CUDA(cudaMemcpyAsync(ctx->d_hx, h_x, nb, cudaMemcpyHostToDevice, st));
+        HT_CUDA(cudaMemcpyAsync(ctx->d_hy, h_y, nb, cudaMemcpyHostToDevice, st));
+        HT_CUDA(cudaMemcpyAsync(ctx->d_hz, h_z, nb, cudaMemcpyHostToDevice, st));
+    }
+    uint32_t *d_count = reinterpret_cast<uint32_t *>(ctx->d_hres);
+    ht_peak *d_list = reinterpret_cast<ht_peak *>(ctx->d_hres + kResHeader);
+    uint32_t found_total = 0u, written = 0u;
+    const int slots = ctx->cfg.host_slots;
+    std::vector<int32_t> off_local((size_t)slots + 1);
+    for (int e0 = 0; e0 < n_events; e0 += slots) {
+        const int ne = (n_events - e0 < slots) ? n_events - e0 : slots;
+        const int32_t hb = h_event_offsets[e0];
+        for (int k = 0; k <= ne; ++k) off_local[(size_t)k] = h_event_offsets[e0 + k] - hb;
+        const int32_t nh = off_local[(size_t)ne];
+        // off_local is reused by the next group: the copy below must have consumed it before we overwrite it,
+        // which the synchronisation at the end of this iteration guarantees.
+        HT_CUDA(cudaMemcpyAsync(ctx->d_hoff, off_local.data(), sizeof(int32_t) * (size_t)(ne + 1), cudaMemcpyHostToDevice, st));
+        int rc = ht_fill(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, st);
+        if (rc == HT_ERR_UNSUPPORTED)
+            rc = ht_fill_naive(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, st);
+        if (rc != HT_OK) return rc;
+        const uint32_t room = capacity - written;
+        rc = ht_peaks(ctx, ctx->d_hmh, ne, threshold, d_list, room, d_count, st);
+        if (rc != HT_OK) return rc;
+        // one D2H for count + a first slice of the list; a second one only if the list is longer than the slice
+        const uint32_t slice = room < 4096u ? room : 4096u;
+        HT_CUDA(cudaMemcpyAsync(ctx->h_res, ctx->d_hres, kResHeader + sizeof(ht_peak) * (size_t)slice, cudaMemcpyDeviceToHost, st));
+        if (h_mh_or_null)
+            HT_CUDA(cudaMemcpyAsync(h_mh_or_null + (size_t)e0 * cells, ctx->d_hmh, sizeof(uint32_t) * cells * (size_t)ne,
+                                    cudaMemcpyDeviceToHost, st));
+        HT_CUDA(cudaStreamSynchronize(st));
+        const uint32_t found = *reinterpret_cast<const uint32_t *>(ctx->h_res);
+        const uint32_t got = found < room ? found : room;
+        if (got > slice) {
+            HT_CUDA(cudaMemcpyAsync(ctx->h_res + kResHeader + sizeof(ht_peak) * (size_t)slice,
+                                    ctx->d_hres + kResHeader + sizeof(ht_peak) * (size_t)slice,
+                                    sizeof(ht_peak) * (size_t)(got - slice), cudaMemcpyDeviceToHost, st));
+            HT_CUDA(cudaStreamSynchronize(st));
+        }
+        const ht_peak *src = reinterpret_cast<const ht_peak *>(ctx->h_res + kResHeader);
+        for (uint32_t k = 0; k < got; ++k) {
+            ht_peak p = src[k];
+            p.event += (uint32_t)e0;
+            h_out[written + k] = p;
+        }
+        written += got;
+        found_total += found;
+    }
+    *h_n_found = found_total;
+    return HT_OK;
+}
+
+int64_t ht_kernel_launches(const ht_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int ht_launch_info(const ht_ctx *ctx, int32_t out[8])
+{
+    if (!ctx || !out) return HT_ERR_INVALID_ARG;
+    std::memcpy(out, ctx->info, sizeof ctx->info);
+    return HT_OK;
+}
+
+void ht_destroy(ht_ctx *ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->cfg.device);
+    if (ctx->host_stream) { cudaStreamSynchronize(ctx->host_stream); cudaStreamDestroy(ctx->host_stream); }
+    cudaFree(ctx->d_rec);
+    cudaFree(ctx->d_plane_off);
+    cudaFree(ctx->d_tth);
+    cudaFree(ctx->d_counters);
+    cudaFree(ctx->d_hx);
+    cudaFree(ctx->d_hoff);
+    cudaFree(ctx->d_hmh);
+    cudaFree(ctx->d_hres);
+    if (ctx->h_res) cudaFreeHost(ctx->h_res);
+    delete ctx;
+}
+
+const char *ht_strerror(int status)
+{
+    switch (status) {
+    case HT_OK: return "ok";
+    case HT_ERR_INVALID_ARG: return "invalid argument";
+    case HT_ERR_UNSUPPORTED: return "binning not supported by the slab kernel (use ht_fill_naive) or call unavailable";
+    case HT_ERR_CUDA: return g_cuda_err;
+    case HT_ERR_NOMEM: return "out of memory";
+    default: return "unknown status";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,263 @@
+"""-m gpu: the CUDA path (through the C-ABI) against the CPU oracle, element by element, on the same seeded inputs.
+
+Bar (BASELINE.json north_star): the vote matrix and the sorted peak list are BIT-EXACT.  Integer work throughout;
+the floating point that decides bin indices is IEEE binary32 on both sides (SPEC.md section 0).
+"""
+import numpy as np
+import pytest
+import torch
+
+from gpu_util import GpuHough, mh_to_numpy, sort_peaks
+from oracle import oracle_fill, oracle_peaks, oracle_peaks_batch
+from paper_1507_03074_b200 import binding as B
+from paper_1507_03074_b200.events import Binning, WORKLOADS, batch_from_arrays, generate_batch
+
+pytestmark = pytest.mark.gpu
+
+
+def _oracle_batch(bn, batch):
+    return [oracle_fill(bn, *batch.event(e))[0] for e in range(batch.n_events)]
+
+
+def _check_batch(bn, batch, threshold, naive=False, capacity=1 << 20):
+    want_m = _oracle_batch(bn, batch)
+    with GpuHough(bn, max_events=max(1, batch.n_events), max_hits=batch.n_hits) as g:
+        mh = g.fill(batch, naive=naive)
+        got = mh_to_numpy(mh, bn, batch.n_events)
+        for e in range(batch.n_events):
+            np.testing.assert_array_equal(got[e], want_m[e], err_msg=f"event {e}")
+        n, pk = g.peaks(mh, batch.n_events, threshold, capacity)
+    want_p = oracle_peaks_batch(bn, want_m, threshold)
+    assert n == len(want_p)
+    if capacity >= n:
+        np.testing.assert_array_equal(sort_peaks(pk, bn.cells), want_p)
+    return n
+
+
+# ------------------------------------------------------------------ the five configs of BASELINE.json
+def test_config1_tiny_three_events():
+    wl = WORKLOADS[1]
+    assert _check_batch(wl.binning, generate_batch(wl, n_events=3), wl.threshold) > 10
+
+
+def test_config2_paper_single_event_full_matrix():
+    wl = WORKLOADS[2]
+    n = _check_batch(wl.binning, generate_batch(wl), wl.threshold)
+    assert 300 < n < 3000
+
+
+def test_config3_batch_of_ragged_events():
+    wl = WORKLOADS[3]
+    batch = generate_batch(wl, n_events=5)
+    assert len(set(np.diff(batch.event_offsets).tolist())) == 5
+    _check_batch(wl.binning, batch, wl.threshold)
+
+
+def test_config4_high_occupancy():
+    wl = WORKLOADS[4]
+    n = _check_batch(wl.binning, generate_batch(wl), wl.threshold)
+    assert n > 5000
+
+
+def test_config5_fine_binning_one_event_full_matrix():
+    wl = WORKLOADS[5]
+    _check_batch(wl.binning, generate_batch(wl, n_events=1), wl.threshold)
+
+
+def test_config5_two_events_sampled():
+    """Two 4.3 GB matrices in one call (64-bit addressing across events): event 1 against the oracle on sampled planes,
+    event 0 via properties (sum == votes)."""
+    wl = WORKLOADS[5]
+    bn = wl.binning
+    batch = generate_batch(wl, n_events=2)
+    with GpuHough(bn, max_events=2, max_hits=batch.n_hits) as g:
+        mh = g.fill(batch)
+        n, pk = g.peaks(mh, 2, wl.threshold)
+        want1, votes1 = oracle_fill(bn, *batch.event(1))
+        m1 = mh[bn.cells:].view(bn.planes, bn.n_a * bn.n_b)
+        for p in (0, 1, 77, 128, 200, 255):
+            np.testing.assert_array_equal(m1[p].cpu().numpy().view(np.uint32),
+                                          want1.reshape(bn.planes, -1)[p])
+        assert int(mh[bn.cells:].sum(dtype=torch.int64)) == votes1
+        want_p1 = oracle_peaks(bn, want1, wl.threshold, event=1)
+        got_p = sort_peaks(pk, bn.cells)
+        np.testing.assert_array_equal(got_p[got_p["event"] == 1], want_p1)
+        assert (got_p["event"] == 0).sum() > 0
+
+
+def test_naive_paper_design_matches_too():
+    wl = WORKLOADS[1]
+    _check_batch(wl.binning, generate_batch(wl, n_events=2), wl.threshold, naive=True)
+    wl = WORKLOADS[2]
+    _check_batch(wl.binning, generate_batch(wl), wl.threshold, naive=True)
+
+
+# ------------------------------------------------------------------ shapes: ragged tiles, odd sizes, partial ranges
+@pytest.mark.parametrize("dims", [(4, 16, 1000, 1024),      # NA not a multiple of the rows per slab: ragged last tile
+                                  (3, 5, 77, 36),            # small, odd plane count, NB % 4 == 0
+                                  (1, 1, 1, 4), (2, 2, 5, 8),
+                                  (4, 16, 37, 4096),         # wide rows: few rows per slab
+                                  (2, 3, 300, 12000)])       # one row = 48 KB: one row per slab
+def test_slab_geometries(dims):
+    bn = Binning(*dims)
+    batch = generate_batch(1, n_events=2)
+    _check_batch(bn, batch, 3)
+
+
+@pytest.mark.parametrize("dims", [(2, 3, 9, 7), (4, 16, 50, 130), (1, 2, 3, 1)])
+def test_shapes_the_slab_kernel_refuses_go_through_the_naive_kernel(dims):
+    bn = Binning(*dims)
+    batch = generate_batch(1)
+    with GpuHough(bn, 1, batch.n_hits) as g:
+        with pytest.raises(B.HtError) as ei:
+            g.fill(batch)
+        assert ei.value.status == B.HT_ERR_UNSUPPORTED
+    _check_batch(bn, batch, 2, naive=True)
+
+
+def test_partial_angle_ranges_and_asymmetric_ab_ranges():
+    bn = Binning(3, 5, 96, 64, a_min=-2500.0, a_max=3100.0, b_min=-700.0, b_max=3900.0,
+                 theta_min=0.6, theta_max=2.2, phi_min=0.5, phi_max=5.5)
+    _check_batch(bn, generate_batch(2), 4)
+
+
+# ------------------------------------------------------------------ degenerate inputs
+def test_empty_and_degenerate_events():
+    bn = WORKLOADS[1].binning
+    ev = generate_batch(1).event(0)
+    good = np.stack(ev, axis=1)
+    bad = np.array([[100.0, 0.0, 5.0], [0.0, 0.0, 1.0], [np.nan, 3.0, 1.0], [3.0, np.nan, 1.0], [3.0, 4.0, np.nan],
+                    [np.inf, 4.0, 1.0], [3.0, -np.inf, 1.0], [-50.0, -0.0, 1.0], [1e-30, 1e-30, 1.0], [1e30, 1e30, 1e30]],
+                   np.float32)
+    batch = batch_from_arrays([np.zeros((0, 3)), good, bad, np.concatenate([bad, good]), np.zeros((0, 3))])
+    _check_batch(bn, batch, 8)
+    # a batch with no hits at all still writes zero matrices
+    empty = batch_from_arrays([np.zeros((0, 3)), np.zeros((0, 3))])
+    with GpuHough(bn, 2, 1) as g:
+        mh = g.fill(empty)
+        assert int(mh.abs().sum()) == 0
+        n, pk = g.peaks(mh, 2, 1)
+        assert n == 0 and len(pk) == 0
+        # zero events: both calls are no-ops that succeed
+        B.ht_fill(g.ctx, None, None, None, None, 0, 0, None)
+        nf = torch.full((1,), 5, dtype=torch.int32, device="cuda")
+        B.ht_peaks(g.ctx, None, 0, 1, None, 0, nf)
+        torch.cuda.synchronize()
+        assert int(nf) == 0
+
+
+def test_all_hits_in_one_plane_many_hits():
+    # 30000 hits in a narrow cone: one plane gets everything (chunked vote loop, counts far above 255)
+    rng = np.random.default_rng(3)
+    n = 30000
+    ph = rng.uniform(0.30, 0.35, n); r = rng.uniform(60, 1000, n)
+    xyz = np.stack([r * np.cos(ph), r * np.sin(ph), r * 0.2], axis=1)
+    bn = Binning(4, 16, 64, 256)
+    batch = batch_from_arrays([xyz])
+    n_pk = _check_batch(bn, batch, 300)
+    assert n_pk > 0
+
+
+# ------------------------------------------------------------------ peaks: hand-built matrices, capacity, thresholds
+def test_peaks_on_hand_built_matrices_from_golden():
+    from golden_io import read_peak_cases
+    for case in read_peak_cases():
+        bn = Binning(*case["dims"])
+        with GpuHough(bn, 1, 1) as g:
+            mh = torch.from_numpy(case["m"].reshape(-1).view(np.int32).copy()).cuda()
+            n, pk = g.peaks(mh, 1, case["T"])
+            assert sorted(pk["cell"].tolist()) == case["peaks"], case["name"]
+            assert n == len(case["peaks"])
+
+
+def test_peaks_dense_random_matrices_and_ties():
+    rng = np.random.default_rng(21)
+    for dims, hi in [((2, 3, 40, 64), 3), ((1, 2, 33, 128), 2), ((2, 2, 17, 20), 6), ((1, 1, 64, 7), 3)]:
+        bn = Binning(*dims)
+        m = rng.integers(0, hi, size=(2,) + dims, dtype=np.uint32)      # two events, many plateaux
+        with GpuHough(bn, 2, 1) as g:
+            mh = torch.from_numpy(m.reshape(-1).view(np.int32).copy()).cuda()
+            for T in (1, hi - 1):
+                n, pk = g.peaks(mh, 2, T)
+                want = oracle_peaks_batch(bn, [m[0], m[1]], T)
+                assert n == len(want)
+                np.testing.assert_array_equal(sort_peaks(pk, bn.cells), want)
+
+
+def test_peak_capacity_overflow_and_threshold_monotonicity():
+    wl = WORKLOADS[1]
+    bn = wl.binning
+    batch = generate_batch(wl, n_events=2)
+    want_m = _oracle_batch(bn, batch)
+    want = oracle_peaks_batch(bn, want_m, 4)
+    with GpuHough(bn, 2, batch.n_hits) as g:
+        mh = g.fill(batch)
+        n, pk = g.peaks(mh, 2, 4, capacity=7)
+        assert n == len(want) > 7 and len(pk) == 7
+        full = set(map(tuple, want.tolist()))
+        assert all(tuple(r) in full for r in pk.tolist()) and len(set(map(tuple, pk.tolist()))) == 7
+        n0, pk0 = g.peaks(mh, 2, 4, capacity=0)
+        assert n0 == len(want)
+        n4, pk4 = g.peaks(mh, 2, 4)
+        n5, pk5 = g.peaks(mh, 2, 5)
+        s4 = sort_peaks(pk4, bn.cells)
+        np.testing.assert_array_equal(sort_peaks(pk5, bn.cells), s4[s4["count"] >= 5])
+        # repeated calls give the same answer (the scratch counters reset themselves)
+        n4b, _ = g.peaks(mh, 2, 4)
+        assert n4b == n4 == len(want)
+
+
+# ------------------------------------------------------------------ streams, repeated calls, host entry point
+def test_fill_on_a_side_stream_and_buffer_reuse():
+    wl = WORKLOADS[1]
+    bn = wl.binning
+    b0, b1 = generate_batch(wl, n_events=1), generate_batch(wl, n_events=1, first_event=1)
+    st = torch.cuda.Stream()
+    with GpuHough(bn, 1, max(b0.n_hits, b1.n_hits)) as g:
+        m0 = mh_to_numpy(g.fill(b0, stream=st), bn, 1)[0]
+        m1 = mh_to_numpy(g.fill(b1, stream=st), bn, 1)[0]
+        np.testing.assert_array_equal(m0, oracle_fill(bn, *b0.event(0))[0])
+        np.testing.assert_array_equal(m1, oracle_fill(bn, *b1.event(0))[0])
+
+
+def test_run_host_end_to_end():
+    wl = WORKLOADS[1]
+    bn = wl.binning
+    batch = generate_batch(wl, n_events=5)
+    want_m = _oracle_batch(bn, batch)
+    want = oracle_peaks_batch(bn, want_m, wl.threshold)
+    with GpuHough(bn, 5, batch.n_hits, host_slots=2, host_peak_capacity=4096) as g:     # 5 events through 2 slots
+        out = np.zeros(4096, B.PEAK_DTYPE)
+        h_mh = np.full(5 * bn.cells, 0xFFFFFFFF, np.uint32)
+        n = B.ht_run_host(g.ctx, batch.x, batch.y, batch.z, batch.event_offsets, 5, batch.n_hits, wl.threshold, out, 4096, h_mh)
+        assert n == len(want)
+        np.testing.assert_array_equal(sort_peaks(out[:n], bn.cells), want)
+        for e in range(5):
+            np.testing.assert_array_equal(h_mh[e * bn.cells:(e + 1) * bn.cells].reshape(want_m[e].shape), want_m[e])
+        # truncated list
+        out2 = np.zeros(3, B.PEAK_DTYPE)
+        n2 = B.ht_run_host(g.ctx, batch.x, batch.y, batch.z, batch.event_offsets, 5, batch.n_hits, wl.threshold, out2, 3)
+        assert n2 == n
+        assert B.ht_kernel_launches(g.ctx) >= 2 * 3 * 3
+
+
+def test_error_codes_on_device_calls():
+    bn = WORKLOADS[1].binning
+    batch = generate_batch(1)
+    with GpuHough(bn, 1, 100) as g:                      # max_hits 100 < 264
+        with pytest.raises(B.HtError) as ei:
+            g.fill(batch)
+        assert ei.value.status == B.HT_ERR_INVALID_ARG
+    with GpuHough(bn, 1, 1000) as g:
+        mh = g.fill(batch)
+        nf = torch.zeros(1, dtype=torch.int32, device="cuda")
+        with pytest.raises(B.HtError):
+            B.ht_peaks(g.ctx, mh, 1, 0, None, 0, nf)     # threshold 0
+        with pytest.raises(B.HtError):
+            B.ht_peaks(g.ctx, mh, 2, 1, None, 0, nf)     # n_events > max_events
+        with pytest.raises(B.HtError) as ei:
+            B.ht_run_host(g.ctx, batch.x, batch.y, batch.z, batch.event_offsets, 1, batch.n_hits, 8, None, 0)
+        assert ei.value.status == B.HT_ERR_UNSUPPORTED   # host_slots == 0
+    cfg = B.ht_config.from_binning(bn, max_events=1, max_hits=1, device=99)
+    with pytest.raises(B.HtError):
+        B.ht_create(cfg)
