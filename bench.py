@@ -147,11 +147,13 @@ def bench_ours(args):
 
     wl = WORKLOADS[args.config]
     bn = wl.binning
-    batch = generate_batch(wl, n_events=1, seed_offset=rank)          # every rank its own event (weak scaling)
+    n_ev = args.events if args.events else 1
+    # every rank its own events (weak scaling: the path shards by event, no data-path collective)
+    batch = generate_batch(wl, n_events=n_ev, first_event=rank * n_ev)
     n_hits = batch.n_hits
     cells = bn.cells
     cap = 1 << 16
-    cfg = B.ht_config.from_binning(bn, max_events=1, max_hits=n_hits, device=local_rank, host_slots=1,
+    cfg = B.ht_config.from_binning(bn, max_events=n_ev, max_hits=n_hits, device=local_rank, host_slots=n_ev,
                                    host_peak_capacity=cap)
     ctx = B.ht_create(cfg)
     stream = torch.cuda.Stream(device=dev)
@@ -159,107 +161,181 @@ def bench_ours(args):
     to = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dtype=dt)
     dx, dy, dz = to(batch.x, torch.float32), to(batch.y, torch.float32), to(batch.z, torch.float32)
     doff = to(batch.event_offsets, torch.int32)
-    n_rot = args.rotate                                               # rotate output matrices: no step inherits L2 contents
-    mhs = [torch.empty(cells, dtype=torch.int32, device=dev) for _ in range(n_rot)]
+    mh_bytes = 4 * cells * n_ev
+    n_rot = args.rotate if mh_bytes * args.rotate <= (8 << 30) else 1   # rotate output matrices: no step inherits L2 contents
+    mhs = [torch.empty(cells * n_ev, dtype=torch.int32, device=dev) for _ in range(n_rot)]
     d_out = torch.empty(cap * 3, dtype=torch.int32, device=dev)
     d_nf = torch.zeros(1, dtype=torch.int32, device=dev)
+    T = wl.threshold
 
-    def step(k, evs=None):
+    def step_fused(k, evs=None):                      # a0-a5 in ONE kernel, matrix materialised
+        if evs is not None:
+            evs[0].record(stream)
+        B.ht_fill_peaks(ctx, dx, dy, dz, doff, n_ev, n_hits, mhs[k % n_rot], T, d_out, cap, d_nf, stream)
+        if evs is not None:
+            evs[1].record(stream)
+
+    def step_split(k, evs=None):                      # the paper's two-kernel split: ht_fill, then ht_peaks
         mh = mhs[k % n_rot]
         if evs is not None:
             evs[0].record(stream)
-        B.ht_fill(ctx, dx, dy, dz, doff, 1, n_hits, mh, stream)
+        B.ht_fill(ctx, dx, dy, dz, doff, n_ev, n_hits, mh, stream)
         if evs is not None:
             evs[1].record(stream)
-        B.ht_peaks(ctx, mh, 1, wl.threshold, d_out, cap, d_nf, stream)
+        B.ht_peaks(ctx, mh, n_ev, T, d_out, cap, d_nf, stream)
         if evs is not None:
             evs[2].record(stream)
 
-    # ---- warm-up, then parity of exactly this launch configuration against the oracle (rank 0)
-    for k in range(max(args.warmup, 3)):
-        step(k)
-    stream.synchronize()
-    n_found = int(d_nf.cpu().numpy().view(np.uint32)[0])
+    def step_nostore(k, evs=None):                    # peaks only: the matrix never leaves shared memory
+        if evs is not None:
+            evs[0].record(stream)
+        B.ht_fill_peaks(ctx, dx, dy, dz, doff, n_ev, n_hits, None, T, d_out, cap, d_nf, stream)
+        if evs is not None:
+            evs[1].record(stream)
 
-    # ---- timed region: K steps back to back; per-call CUDA events on the launch stream
     def barrier():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    def n_found_now():
+        stream.synchronize()
+        return int(d_nf.cpu().numpy().view(np.uint32)[0])
+
+    def timed(step, n_marks, sampler=None):
+        """W warm-up steps, then exactly K steps bracketed by barrier+synchronize; CUDA events on the launch stream."""
+        for k in range(max(args.warmup, 3)):
+            step(k)
+        found = n_found_now()
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(n_marks)] for _ in range(args.steps)]
+        l0 = B.ht_kernel_launches(ctx)
+        barrier()
+        if sampler is not None:
+            sampler.start()
+        t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t_start.record(stream)
+        for k in range(args.steps):
+            step(k, evs[k])
+        t_end.record(stream)
+        barrier()
+        if sampler is not None:
+            sampler.stop_flag = True
+        launches = B.ht_kernel_launches(ctx) - l0
+        total_ms = t_start.elapsed_time(t_end)
+        if world > 1:
+            t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            total_ms = float(t.item())
+        spans = [[e[i].elapsed_time(e[i + 1]) for e in evs] for i in range(n_marks - 1)]
+        return total_ms / args.steps, spans, launches, found
+
+    fused_ok = True
+    try:
+        step_fused(0)
+        stream.synchronize()
+    except B.HtError as err:
+        if err.status != B.HT_ERR_UNSUPPORTED:
+            raise
+        fused_ok = False
+    headline = "fused" if (fused_ok and args.mode != "split") else "split"
+
     sampler = ClockSampler(local_rank)
-    launches0 = B.ht_kernel_launches(ctx)
-    barrier()
-    sampler.start()
-    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_start.record(stream)
-    for k in range(args.steps):
-        step(k, evs[k])
-    t_end.record(stream)
-    barrier()
-    sampler.stop_flag = True
-    launches = B.ht_kernel_launches(ctx) - launches0
-    total_ms = t_start.elapsed_time(t_end)
-    fill_ms = [e[0].elapsed_time(e[1]) for e in evs]
-    peaks_ms = [e[1].elapsed_time(e[2]) for e in evs]
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    ms_per_step = total_ms / args.steps
-    value = world * 1e3 / ms_per_step                                 # events/s over all ranks
+    res = {}
+    if headline == "fused":
+        res["fused"] = timed(step_fused, 2, sampler)
+        res["split"] = timed(step_split, 3)
+    else:
+        res["split"] = timed(step_split, 3, sampler)
+        if fused_ok:
+            res["fused"] = timed(step_fused, 2)
+    if fused_ok:
+        res["nostore"] = timed(step_nostore, 2)
+    # leave the headline path's outputs in the buffers for the parity check below
+    last_k = args.steps - 1
+    (step_fused if headline == "fused" else step_split)(last_k)
+    n_found = n_found_now()
+    ms_per_step, _, launches, _ = res[headline]
+    value = world * n_ev * 1e3 / ms_per_step                          # events/s over all ranks
 
     # ---- end to end through the host entry point: pinned host buffers, H2D + D2H inside the timed region
     hx, hy, hz = (torch.from_numpy(a.copy()).pin_memory() for a in (batch.x, batch.y, batch.z))
     hoff = torch.from_numpy(batch.event_offsets.copy()).pin_memory()
     hout = torch.zeros(cap * 3, dtype=torch.int32).pin_memory()
     for _ in range(3):
-        n_e2e = B.ht_run_host(ctx, hx, hy, hz, hoff, 1, n_hits, wl.threshold, hout, cap)
+        n_e2e = B.ht_run_host(ctx, hx, hy, hz, hoff, n_ev, n_hits, T, hout, cap)
     barrier()
     e2e_steps = args.steps
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        n_e2e = B.ht_run_host(ctx, hx, hy, hz, hoff, 1, n_hits, wl.threshold, hout, cap)
+        n_e2e = B.ht_run_host(ctx, hx, hy, hz, hoff, n_ev, n_hits, T, hout, cap)
     e2e_s = time.perf_counter() - t0
     if world > 1:
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
-    e2e_value = world * e2e_steps / e2e_s
-    h2d = 3 * 4 * n_hits + 4 * 2
-    d2h = 16 + 12 * min(cap, 4096)
+    e2e_value = world * n_ev * e2e_steps / e2e_s
+    h2d = 3 * 4 * n_hits + 4 * (n_ev + 1)
+    d2h = 16 + 12 * min(cap, 1024)
 
     if rank == 0:
         peak_gbs, peak_src = measured_hbm_peak()
-        fill_med, peaks_med = statistics.median(fill_ms), statistics.median(peaks_ms)
-        fill_avg, peaks_avg = sum(fill_ms) / len(fill_ms), sum(peaks_ms) / len(peaks_ms)
-        mh_bytes = 4 * cells
-        fill_bytes = mh_bytes + 12 * n_hits        # store every cell once + read the hits
-        peaks_bytes = mh_bytes + 12 * n_found      # read every cell once + write the peak list
-        roof = {}
-        for name, nbytes, avg in (("ht_fill (classify_bucket + fill_slab)", fill_bytes, fill_avg),
-                                  ("ht_peaks (peaks_kernel)", peaks_bytes, peaks_avg)):
-            ach = nbytes / (avg * 1e-3) / 1e9
-            roof[name] = {"bound": "hbm", "achieved": ach, "peak": peak_gbs, "unit": "GB/s", "frac": ach / peak_gbs,
-                          "traffic": None, "kernel": name, "algorithmic_bytes_per_launch": nbytes,
-                          "avg_ms_per_launch": avg, "peak_source": peak_src}
-        dominant = max(roof.values(), key=lambda r: r["avg_ms_per_launch"])
-        other = min(roof.values(), key=lambda r: r["avg_ms_per_launch"])
+        mean = lambda v: sum(v) / len(v)
+        m_bytes = 4 * cells * n_ev
+        hit_bytes, pk_bytes = 12 * n_hits, 12 * n_found
 
-        # ---- cpu_baseline (oracle, 1 core) on the same event + parity of this very launch configuration
-        reps = 3
-        o_times = []
+        def roof(name, nbytes, ms):
+            ach = nbytes / (ms * 1e-3) / 1e9
+            return {"bound": "hbm", "achieved": ach, "peak": peak_gbs, "unit": "GB/s", "frac": ach / peak_gbs,
+                    "traffic": None, "kernel": name, "algorithmic_bytes_per_launch": nbytes, "avg_ms_per_launch": ms,
+                    "peak_source": peak_src}
+
+        kernels, kernel_ms = {}, {}
+        if "fused" in res:
+            f = res["fused"][1][0]
+            kernels["ht_fill_peaks"] = roof("fill_stream_kernel<true> (ht_fill_peaks: classify+vote+store+peak test+compaction)",
+                                            m_bytes + hit_bytes + pk_bytes, mean(f))
+            kernel_ms.update(fused_median=statistics.median(f), fused_mean=mean(f), fused_step_mean=res["fused"][0])
+        sp_fill, sp_peaks = res["split"][1]
+        kernels["ht_fill"] = roof("fill_stream_kernel<false> (ht_fill: classify+vote+store)", m_bytes + hit_bytes, mean(sp_fill))
+        kernels["ht_peaks"] = roof("peaks_kernel (ht_peaks: scan+compaction)", m_bytes + pk_bytes, mean(sp_peaks))
+        kernel_ms.update(fill_median=statistics.median(sp_fill), fill_mean=mean(sp_fill),
+                         peaks_median=statistics.median(sp_peaks), peaks_mean=mean(sp_peaks),
+                         split_step_mean=res["split"][0])
+        if "nostore" in res:
+            kernel_ms.update(nostore_median=statistics.median(res["nostore"][1][0]), nostore_step_mean=res["nostore"][0])
+        if headline == "fused":
+            dominant = kernels["ht_fill_peaks"]
+        else:
+            dominant = max((kernels["ht_fill"], kernels["ht_peaks"]), key=lambda r: r["avg_ms_per_launch"])
+
+        # ---- cpu_baseline (oracle, 1 core) on event 0 + parity of this very launch configuration
+        from oracle import oracle_fill, oracle_peaks
+        reps, o_times, votes = 3, [], 0
         for _ in range(reps):
-            m_ref, pk_ref, votes, tf, tp = run_oracle_event(bn, batch, wl.threshold)
+            m_ref, pk_ref, votes, tf, tp = run_oracle_event(bn, batch, T)
             o_times.append((tf, tp))
-        got_m = mhs[(args.steps - 1) % n_rot].cpu().numpy().view(np.uint32).reshape(m_ref.shape)
+        got_all = mhs[last_k % n_rot].cpu().numpy().view(np.uint32).reshape(n_ev, -1)
         k = min(n_found, cap)
         rec = d_out[:3 * k].cpu().numpy().view(np.uint32).reshape(k, 3)
-        order = np.argsort(rec[:, 1].astype(np.int64), kind="stable")
-        parity = bool(np.array_equal(got_m, m_ref) and n_found == len(pk_ref) and n_e2e == len(pk_ref)
-                      and np.array_equal(rec[order, 1], pk_ref["cell"]) and np.array_equal(rec[order, 2], pk_ref["count"]))
+        rec = rec[np.lexsort((rec[:, 1], rec[:, 0]))]
+        parity = bool(np.array_equal(got_all[0], m_ref.reshape(-1)))
+        n_ref, votes_all = 0, 0
+        for e in range(n_ev):
+            if e == 0:
+                m_e, pk_e, v_e = m_ref, pk_ref, votes
+            else:
+                m_e, v_e = oracle_fill(bn, *batch.event(e))
+                pk_e = oracle_peaks(bn, m_e, T)
+                parity = parity and bool(np.array_equal(got_all[e], m_e.reshape(-1)))
+            votes_all += v_e
+            r_e = rec[rec[:, 0] == e]
+            parity = parity and len(r_e) == len(pk_e) and bool(np.array_equal(r_e[:, 1], pk_e["cell"])
+                                                                and np.array_equal(r_e[:, 2], pk_e["count"]))
+            n_ref += len(pk_e)
+        parity = parity and n_found == n_ref and n_e2e == n_ref
+        for name in res:
+            parity = parity and res[name][3] == n_ref
         o_fill = statistics.median(t[0] for t in o_times)
         o_peaks = statistics.median(t[1] for t in o_times)
         info = B.ht_launch_info(ctx)
@@ -268,18 +344,20 @@ def bench_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u32 counts / f32 bin decisions", "data": "synthetic",
             "config": {"workload": f"config{wl.config}:{wl.name}", "bins": [bn.n_theta, bn.n_phi, bn.n_a, bn.n_b],
-                       "hits_per_event": n_hits, "threshold": wl.threshold, "events_per_step": 1,
-                       "l2": f"M_H per event ({mh_bytes / 1e6:.0f} MB) vs 126 MB L2; {n_rot} output matrices rotated so "
-                             "no step inherits another step's lines",
+                       "hits_per_step": n_hits, "threshold": T, "events_per_step": n_ev,
+                       "path": ("ht_fill_peaks: one kernel does a0-a5 and stores every M_H cell once" if headline == "fused"
+                                else "ht_fill + ht_peaks (two kernels)"),
+                       "l2": f"M_H per step ({m_bytes / 1e6:.0f} MB) is larger than the 126 MB L2; {n_rot} output matrices "
+                             "rotated so no step inherits another step's lines",
                        "launch": info},
-            "votes_per_s": votes * value, "votes_per_event": votes, "peaks_per_event": n_found,
-            "hit_a_evaluations_per_s": n_hits * bn.n_a * value,
+            "votes_per_s": votes_all * world * 1e3 / ms_per_step, "votes_per_step": votes_all, "peaks_per_step": n_found,
+            "hit_a_evaluations_per_s": n_hits * bn.n_a * world * 1e3 / ms_per_step,
             "parity_vs_oracle": "bit-exact" if parity else "MISMATCH",
-            "kernel_ms": {"fill_median": fill_med, "fill_mean": fill_avg, "peaks_median": peaks_med,
-                          "peaks_mean": peaks_avg, "step_mean": ms_per_step},
-            "roofline": dominant, "roofline_other": other,
+            "kernel_ms": kernel_ms,
+            "paths_events_per_s": {name: world * n_ev * 1e3 / r[0] for name, r in res.items()},
+            "roofline": dominant, "roofline_kernels": kernels,
             "cpu_baseline": {"value": 1.0 / (o_fill + o_peaks), "unit": "events/s", "cores": 1, "kind": "oracle",
-                             "sample": f"median of {reps} runs of the same full event (fill {o_fill * 1e3:.0f} ms + "
+                             "sample": f"median of {reps} runs of one full event of this workload (fill {o_fill * 1e3:.0f} ms + "
                                        f"peaks {o_peaks * 1e3:.0f} ms), single thread, host of the GPU box",
                              "host_cpus": os.cpu_count()},
             "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -303,7 +381,10 @@ def main():
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 4])
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--events", type=int, default=0, help="events per step (default 1)")
+    ap.add_argument("--mode", choices=["fused", "split"], default="fused",
+                    help="headline path: ht_fill_peaks (one kernel) or ht_fill + ht_peaks")
     ap.add_argument("--rotate", type=int, default=4, help="number of output matrices rotated between steps")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -14,12 +14,11 @@
  *
  * Conventions
  *   - Pointers named d_* are DEVICE pointers (on cfg.device), h_* are HOST pointers.  The caller owns every
- *     buffer it passes; the library owns only the ht_ctx (host struct + small device workspace: tables,
- *     bucketed hits, per-(event,plane) offsets, counters; and, if cfg.host_slots > 0, staging buffers
- *     and host_slots vote matrices for ht_run_host).
+ *     buffer it passes; the library owns only the ht_ctx (host struct + small device workspace: the angle tables
+ *     and two counters; and, if cfg.host_slots > 0, staging buffers and host_slots vote matrices for ht_run_host).
  *   - Layout of a vote matrix (R15): uint32 M[event][itheta][iphi][ia][ib], ib fastest;
  *     cell = ((itheta*Nphi + iphi)*NA + ia)*NB + ib  (< 2^32 required).  d_mh must be 16-byte aligned.
- *   - ht_fill / ht_fill_naive / ht_peaks only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
+ *   - ht_fill / ht_fill_peaks / ht_fill_naive / ht_peaks only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
  *     void*, e.g. torch.cuda.Stream().cuda_stream; NULL = the legacy default stream).  No host
  *     synchronisation, no allocation.  Results are valid once the caller has synchronised the stream.
  *     Calls on one context must be stream-ordered with respect to each other (a context is not
@@ -47,7 +46,7 @@ typedef enum ht_status {
     HT_OK = 0,
     HT_ERR_INVALID_ARG = -1, /* null pointer, non-positive bins, min >= max, non-finite range, n_events > max_events,
                                 n_hits_total > max_hits, threshold == 0, cells >= 2^32 */
-    HT_ERR_UNSUPPORTED = -2, /* binning does not fit the slab kernel (see ht_fill) -- use ht_fill_naive */
+    HT_ERR_UNSUPPORTED = -2, /* binning does not fit the kernel (see ht_fill, ht_fill_peaks), or call unavailable */
     HT_ERR_CUDA = -3,        /* a CUDA runtime call or a launch failed */
     HT_ERR_NOMEM = -4        /* host or device allocation failed */
 } ht_status;
@@ -90,16 +89,32 @@ HT_API int ht_create(const ht_config *cfg, ht_ctx **out);
  *   d_x, d_y, d_z     device, float32 SoA, n_hits_total entries (mm); hits of event e are
  *                     [d_event_offsets[e], d_event_offsets[e+1])
  *   d_event_offsets   device, int32, n_events+1 entries, ascending, first 0, last n_hits_total
- *   n_events, n_hits_total  host copies of the sizes (grid sizing); n_events may be 0 (no-op)
+ *   n_events, n_hits_total  host copies of the sizes (validation, grid sizing); n_events may be 0 (no-op)
  *   d_mh              device, n_events * cells uint32, FULLY OVERWRITTEN: every cell is stored exactly once
- *                     (zero or its count); it need not be cleared beforehand.
- * Kernels: classify+bucket hits by (event, plane); then each CTA builds (plane, A-tile) slabs as private
- * shared-memory histograms and writes them with bulk (TMA) stores: no global atomics, no memset pass.
- * HT_ERR_UNSUPPORTED if n_b % 4 != 0, one A row (n_b*4 bytes) exceeds the slab budget, or planes > 8192.
+ *                     (zero or its count); it need not be cleared beforehand.  4-byte aligned; 16-byte alignment
+ *                     (and n_b % 4 == 0) lets the rows leave as bulk (TMA) stores, otherwise plain stores are used.
+ * One persistent kernel: each CTA owns a contiguous run of A rows of the batch, selects the hits of the current
+ * (event, theta, phi) plane itself, builds tiles of rows as private shared-memory histograms and stores each tile
+ * once: no global atomics, no memset pass, no workspace.
+ * HT_ERR_UNSUPPORTED if one A row (n_b*4 bytes) does not fit the shared-memory tile (n_b > ~12000): ht_fill_naive.
  */
 HT_API int ht_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z,
                    const int32_t *d_event_offsets, int32_t n_events, int32_t n_hits_total, uint32_t *d_mh,
                    void *cuda_stream);
+
+/*
+ * Fill AND peak search in one pass: the same kernel as ht_fill applies the threshold +
+ * local-maximum rule of ht_peaks to each tile while it is still in shared memory, so the matrix is never read back.
+ * The two-kernel split is the paper's ("splitting the code in two kernels"), not a requirement of the
+ * method; results are identical to ht_fill followed by ht_peaks.
+ *   d_mh_or_null      as d_mh of ht_fill, or NULL: the matrices are not materialised at all (peaks only)
+ *   threshold, d_out, capacity, d_n_found   as for ht_peaks
+ * HT_ERR_UNSUPPORTED where ht_fill is, and if fewer than 2 A rows fit a tile (n_b > ~6000): use ht_fill + ht_peaks.
+ */
+HT_API int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z,
+                         const int32_t *d_event_offsets, int32_t n_events, int32_t n_hits_total,
+                         uint32_t *d_mh_or_null, uint32_t threshold, ht_peak *d_out, uint32_t capacity,
+                         uint32_t *d_n_found, void *cuda_stream);
 
 /* The paper's own design (cudaMemset, one block per hit, threads over A, global atomicAdd),
  * same arguments and result as ht_fill, any binning.  Kept as the prior-art comparison and for shapes ht_fill
@@ -120,9 +135,9 @@ HT_API int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_
                     uint32_t capacity, uint32_t *d_n_found, void *cuda_stream);
 
 /*
- * End-to-end call with HOST buffers (needs cfg.host_slots >= 1): copies the hits to the device, runs ht_fill and
- * ht_peaks on the context's own matrices (events in groups of host_slots), copies the peak list and count back
- * and synchronises.  h_out receives min(*h_n_found, capacity) records; capacity <= cfg.host_peak_capacity.
+ * End-to-end call with HOST buffers (needs cfg.host_slots >= 1): copies the hits to the device, runs ht_fill_peaks
+ * (or ht_fill + ht_peaks where that is unsupported) on the context's own matrices (events in groups of host_slots),
+ * copies the peak list and count back and synchronises.  h_out receives min(*h_n_found, capacity) records; capacity <= cfg.host_peak_capacity.
  * h_mh_or_null: if not NULL, n_events * cells uint32 that also receive the matrices (testing; slow).
  * Host buffers may be pageable or pinned (pinned makes the copies asynchronous DMA).
  */
@@ -134,7 +149,7 @@ HT_API int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const fl
 HT_API int64_t ht_kernel_launches(const ht_ctx *ctx);
 
 /* Launch geometry of the last ht_fill / ht_peaks (for DESIGN.md / bench reporting): out[0]=fill grid, out[1]=fill block,
- * out[2]=fill dynamic smem bytes, out[3]=rows per slab, out[4]=peaks grid, out[5]=peaks block, out[6]=SM count, out[7]=0. */
+ * out[2]=fill dynamic smem bytes, out[3]=rows per tile, out[4]=peaks grid, out[5]=peaks block, out[6]=SM count, out[7]=0. */
 HT_API int ht_launch_info(const ht_ctx *ctx, int32_t out[8]);
 
 /* Free everything the context owns.  NULL is allowed. */

@@ -18,7 +18,7 @@ HT_OK, HT_ERR_INVALID_ARG, HT_ERR_UNSUPPORTED, HT_ERR_CUDA, HT_ERR_NOMEM = 0, -1
 
 PEAK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32)])   # == struct ht_peak
 
-EXPORTS = ("ht_query_sizes", "ht_tables_host", "ht_create", "ht_fill", "ht_fill_naive", "ht_peaks", "ht_run_host",
+EXPORTS = ("ht_query_sizes", "ht_tables_host", "ht_create", "ht_fill", "ht_fill_peaks", "ht_fill_naive", "ht_peaks", "ht_run_host",
            "ht_kernel_launches", "ht_launch_info", "ht_destroy", "ht_strerror")
 
 
@@ -70,6 +70,8 @@ def load() -> C.CDLL:
         fn = getattr(lib, name)
         fn.restype = C.c_int
         fn.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, vp]
+    lib.ht_fill_peaks.restype = C.c_int
+    lib.ht_fill_peaks.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, u32, vp, u32, vp, vp]
     lib.ht_peaks.restype = C.c_int
     lib.ht_peaks.argtypes = [vp, vp, i32, u32, vp, u32, vp, vp]
     lib.ht_run_host.restype = C.c_int
@@ -143,6 +145,14 @@ def ht_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events: int, n_hits_total: in
                           _ptr(d_mh), _stream(stream)), "ht_fill")
 
 
+def ht_fill_peaks(ctx, d_x, d_y, d_z, d_event_offsets, n_events: int, n_hits_total: int, d_mh, threshold: int, d_out,
+                  capacity: int, d_n_found, stream=None) -> None:
+    """Fill and peak search in one pass; ``d_mh`` may be None (matrices not materialised)."""
+    _check(load().ht_fill_peaks(ctx, _ptr(d_x), _ptr(d_y), _ptr(d_z), _ptr(d_event_offsets), n_events, n_hits_total,
+                                _ptr(d_mh), threshold, _ptr(d_out), capacity, _ptr(d_n_found), _stream(stream)),
+           "ht_fill_peaks")
+
+
 def ht_fill_naive(ctx, d_x, d_y, d_z, d_event_offsets, n_events: int, n_hits_total: int, d_mh, stream=None) -> None:
     _check(load().ht_fill_naive(ctx, _ptr(d_x), _ptr(d_y), _ptr(d_z), _ptr(d_event_offsets), n_events, n_hits_total,
                                 _ptr(d_mh), _stream(stream)), "ht_fill_naive")
@@ -170,7 +180,7 @@ def ht_kernel_launches(ctx) -> int:
 def ht_launch_info(ctx) -> dict:
     arr = (C.c_int32 * 8)()
     _check(load().ht_launch_info(ctx, C.byref(arr)), "ht_launch_info")
-    keys = ("fill_grid", "fill_block", "fill_smem_bytes", "rows_per_slab", "peaks_grid", "peaks_block", "sm_count")
+    keys = ("fill_grid", "fill_block", "fill_smem_bytes", "rows_per_tile", "peaks_grid", "peaks_block", "sm_count")
     return dict(zip(keys, list(arr)[:7]))
 
 

@@ -101,20 +101,21 @@ struct ht_ctx {
     int max_smem_optin = 0;
     // device workspace
     float *d_tth = nullptr, *d_pph = nullptr;
-    ht::HitRec *d_rec = nullptr;
-    int32_t *d_plane_off = nullptr;
     uint32_t *d_counters = nullptr;
-    // slab-fill launch geometry
+    // row-stream fill launch geometry
     bool slab_ok = false;
-    int rows_per_slab = 0, tiles_per_plane = 0, fill_threads = 0, fill_nbuf = 0, fill_ctas_per_sm = 0;
-    size_t slab_bytes = 0, fill_smem = 0, classify_smem = 0;
-    int peaks_ctas_per_sm = 0;
+    int rows_per_tile = 0, hit_cap = 0, fill_ctas_per_sm = 0;
+    uint32_t slab_words = 0;
+    size_t fill_smem = 0;
+    // peak scan launch geometry
+    int peaks_unroll = 4, peaks_grid_vec4 = 0, peaks_grid_vec1 = 0;
     // host path (ht_run_host)
     float *d_hx = nullptr, *d_hy = nullptr, *d_hz = nullptr;
     int32_t *d_hoff = nullptr;
     uint32_t *d_hmh = nullptr;
     unsigned char *d_hres = nullptr;   // [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
     unsigned char *h_res = nullptr;    // pinned mirror of d_hres
+    int32_t *h_off = nullptr;          // pinned staging of the per-group offsets
     cudaStream_t host_stream = nullptr;
     int64_t launches = 0;
     int32_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -125,7 +126,7 @@ namespace {
 constexpr size_t kResHeader = 16;
 
 struct WorkspaceSizes {
-    size_t rec, plane_off, tables, counters, host_hits, host_off, host_mh, host_res, total;
+    size_t tables, counters, host_hits, host_off, host_mh, host_res, total;
 };
 
 WorkspaceSizes workspace_sizes(const ht_config *c)
@@ -133,8 +134,6 @@ WorkspaceSizes workspace_sizes(const ht_config *c)
     WorkspaceSizes w{};
     const size_t planes = (size_t)c->n_theta * (size_t)c->n_phi;
     const size_t cells = planes * (size_t)c->n_a * (size_t)c->n_b;
-    w.rec = align_up(sizeof(ht::HitRec) * (size_t)c->max_hits, 256);
-    w.plane_off = align_up(sizeof(int32_t) * (size_t)c->max_events * (planes + 1), 256);
     w.tables = align_up(sizeof(float) * (size_t)(c->n_theta + 1 + c->n_phi + 1), 256);
     w.counters = 256;
     if (c->host_slots > 0) {
@@ -143,49 +142,61 @@ WorkspaceSizes workspace_sizes(const ht_config *c)
         w.host_mh = align_up(cells * sizeof(uint32_t) * (size_t)c->host_slots, 256);
         w.host_res = align_up(kResHeader + sizeof(ht_peak) * (size_t)c->host_peak_capacity, 256);
     }
-    w.total = w.rec + w.plane_off + w.tables + w.counters + w.host_hits + w.host_off + w.host_mh + w.host_res;
+    w.total = w.tables + w.counters + w.host_hits + w.host_off + w.host_mh + w.host_res;
     return w;
 }
 
-// Slab geometry: rows per slab so that NBUF slabs of rows*NB*4 bytes fit `ctas_per_sm` CTAs into shared memory.
+// hit_in_plane() (one interval test per angle) equals the count-of-edges rule of SPEC.md section 2 only for monotone
+// tables; they are monotone for every valid configuration (cot and the pseudo-angle are monotone, rounding keeps that).
+bool tables_monotone(const std::vector<float> &tth, const std::vector<float> &pph)
+{
+    for (size_t k = 1; k < tth.size(); ++k)
+        if (!(tth[k] <= tth[k - 1])) return false;
+    for (size_t k = 1; k < pph.size(); ++k)
+        if (!(pph[k] >= pph[k - 1])) return false;
+    return true;
+}
+
+// Tile geometry of the row-stream fill: R rows per slab so that two slabs, the hit list and the row table of
+// `ctas_per_sm` CTAs fit the SM's shared memory.
 void plan_fill(ht_ctx *ctx)
 {
     const ht_config &c = ctx->cfg;
     ctx->slab_ok = false;
     const size_t row_bytes = (size_t)c.n_b * 4u;
     const int slab_kb = env_int("HT_FILL_SLAB_KB", 48);
-    const int nbuf = env_int("HT_FILL_NBUF", 2);
-    const int threads = env_int("HT_FILL_THREADS", 512);
-    const int ctas = env_int("HT_FILL_CTAS_PER_SM", 2);
-    if (nbuf != 1 && nbuf != 2) return;
-    if (threads < 32 || threads > 1024 || (threads & 31)) return;
-    if (c.n_b % 4 != 0) return;
-    if ((long long)c.n_theta * c.n_phi > 8192) return;
-    const size_t budget = (size_t)slab_kb * 1024u;
-    if (row_bytes > budget || (size_t)nbuf * row_bytes > (size_t)ctx->max_smem_optin) return;
-    int rows = (int)(budget / row_bytes);
+    int ctas = env_int("HT_FILL_CTAS_PER_SM", 2);
+    int cap = env_int("HT_FILL_HIT_CAP", 1024);
+    if (ctas < 1) ctas = 1;
+    if (ctas > 2) ctas = 2;                                   // __launch_bounds__(kFillThreads, 2)
+    cap = (cap + ht::kFillThreads - 1) / ht::kFillThreads * ht::kFillThreads;
+    if (cap < ht::kFillThreads) cap = ht::kFillThreads;
+    size_t budget = ((size_t)228 * 1024 - (size_t)ctas * 1024) / (size_t)ctas - 256;    // 1 KB per CTA is reserved; 256: static smem
+    if (budget > (size_t)ctx->max_smem_optin) budget = (size_t)ctx->max_smem_optin;
+    const size_t fixed = 12u * (size_t)cap;
+    long long rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
     if (rows > c.n_a) rows = c.n_a;
-    while (rows > 1 && (size_t)nbuf * (size_t)rows * row_bytes > (size_t)ctx->max_smem_optin) --rows;
-    ctx->rows_per_slab = rows;
-    ctx->tiles_per_plane = (c.n_a + rows - 1) / rows;
-    ctx->slab_bytes = (size_t)rows * row_bytes;
-    ctx->fill_nbuf = nbuf;
-    ctx->fill_threads = threads;
-    ctx->fill_ctas_per_sm = ctas < 1 ? 1 : ctas;
-    ctx->fill_smem = (size_t)nbuf * ctx->slab_bytes;
+    auto need = [&](long long r) { return 2u * align_up((size_t)r * row_bytes, 16) + fixed + align_up(4u * (size_t)r, 16); };
+    while (rows >= 1 && need(rows) > budget) --rows;
+    if (rows < 1) return;                                      // one row does not fit: ht_fill_naive only
+    ctx->rows_per_tile = (int)rows;
+    ctx->hit_cap = cap;
+    ctx->slab_words = (uint32_t)(align_up((size_t)rows * row_bytes, 16) / 4u);
+    ctx->fill_ctas_per_sm = ctas;
+    ctx->fill_smem = need(rows);
     ctx->slab_ok = true;
 }
 
 int check_fill_args(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off,
-                    int32_t n_events, int32_t n_hits_total, uint32_t *d_mh)
+                    int32_t n_events, int32_t n_hits_total, uint32_t *d_mh, bool mh_required)
 {
     if (!ctx) return HT_ERR_INVALID_ARG;
     if (n_events < 0 || n_hits_total < 0) return HT_ERR_INVALID_ARG;
     if (n_events > ctx->cfg.max_events || n_hits_total > ctx->cfg.max_hits) return HT_ERR_INVALID_ARG;
     if (n_events == 0) return HT_OK;
-    if (!d_off || !d_mh) return HT_ERR_INVALID_ARG;
+    if (!d_off || (mh_required && !d_mh)) return HT_ERR_INVALID_ARG;
     if (n_hits_total > 0 && (!d_x || !d_y || !d_z)) return HT_ERR_INVALID_ARG;
-    if ((reinterpret_cast<uintptr_t>(d_mh) & 15u) != 0) return HT_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_mh) & 3u) != 0) return HT_ERR_INVALID_ARG;
     return HT_OK;
 }
 
@@ -213,6 +224,7 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
 {
     if (!out) return HT_ERR_INVALID_ARG;
     if (!config_ok(cfg) || cfg->max_events < 1 || cfg->max_hits < 1 || cfg->host_slots < 0) return HT_ERR_INVALID_ARG;
+    if (cfg->max_hits > INT32_MAX - 65536) return HT_ERR_INVALID_ARG;
     int ndev = 0;
     HT_CUDA(cudaGetDeviceCount(&ndev));
     if (cfg->device < 0 || cfg->device >= ndev) return HT_ERR_INVALID_ARG;
@@ -249,8 +261,6 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
         }
         return true;
     };
-    if (!dmalloc((void **)&ctx->d_rec, w.rec, "cudaMalloc(rec)")) return fail(rc);
-    if (!dmalloc((void **)&ctx->d_plane_off, w.plane_off, "cudaMalloc(plane_off)")) return fail(rc);
     if (!dmalloc((void **)&ctx->d_tth, w.tables, "cudaMalloc(tables)")) return fail(rc);
     ctx->d_pph = ctx->d_tth + (cfg->n_theta + 1);
     if (!dmalloc((void **)&ctx->d_counters, w.counters, "cudaMalloc(counters)")) return fail(rc);
@@ -269,66 +279,117 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
         if (!dmalloc((void **)&ctx->d_hres, w.host_res, "cudaMalloc(host result)")) return fail(rc);
         if ((e = cudaMallocHost((void **)&ctx->h_res, w.host_res)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaMallocHost(result)"));
+        if ((e = cudaMallocHost((void **)&ctx->h_off, w.host_off)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaMallocHost(offsets)"));
         if ((e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaStreamCreate"));
     }
 
     plan_fill(ctx);
-    ctx->classify_smem = sizeof(float) * (size_t)(cfg->n_theta + cfg->n_phi + 2) + sizeof(int) * (2 * (size_t)g.planes + 32);
+    if (ctx->slab_ok && !tables_monotone(tth, pph)) ctx->slab_ok = false;
     if (ctx->slab_ok) {
-        if (ctx->classify_smem > (size_t)ctx->max_smem_optin) ctx->slab_ok = false;
-    }
-    if (ctx->slab_ok) {
-        if ((e = cudaFuncSetAttribute(ht::classify_bucket_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)ctx->classify_smem)) != cudaSuccess ||
-            (e = cudaFuncSetAttribute(ht::fill_slab_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        if ((e = cudaFuncSetAttribute(ht::fill_stream_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)ctx->fill_smem)) != cudaSuccess ||
-            (e = cudaFuncSetAttribute(ht::fill_slab_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+            (e = cudaFuncSetAttribute(ht::fill_stream_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)ctx->fill_smem)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaFuncSetAttribute"));
     }
-    ctx->peaks_ctas_per_sm = env_int("HT_PEAKS_CTAS_PER_SM", 8);
-    if (ctx->peaks_ctas_per_sm < 1) ctx->peaks_ctas_per_sm = 1;
+    // peak scan: a persistent grid of exactly the CTAs that are resident at once (a grid-stride loop over more CTAs
+    // than fit would run the excess as a second, partly empty wave)
+    int unroll = env_int("HT_PEAKS_UNROLL", 4);
+    if (unroll != 2 && unroll != 4 && unroll != 8) unroll = 4;
+    ctx->peaks_unroll = unroll;
+    int occ4 = 0, occ1 = 0;
+    if (unroll == 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ4, ht::peaks_kernel<4, 2>, ht::kPeaksThreads, 0);
+    else if (unroll == 8) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ4, ht::peaks_kernel<4, 8>, ht::kPeaksThreads, 0);
+    else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ4, ht::peaks_kernel<4, 4>, ht::kPeaksThreads, 0);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, ht::peaks_kernel<1, 4>, ht::kPeaksThreads, 0);
+    if (e != cudaSuccess) return fail(cuda_fail(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor"));
+    const int occ_cap = env_int("HT_PEAKS_CTAS_PER_SM", 32);
+    if (occ4 > occ_cap) occ4 = occ_cap;
+    if (occ1 > occ_cap) occ1 = occ_cap;
+    if (occ4 < 1) occ4 = 1;
+    if (occ1 < 1) occ1 = 1;
+    ctx->peaks_grid_vec4 = ctx->sm_count * occ4;
+    ctx->peaks_grid_vec1 = ctx->sm_count * occ1;
     ctx->info[6] = ctx->sm_count;
     *out = ctx;
     return HT_OK;
 }
 
+namespace {
+
+// Launch of the row-stream kernel, with (PEAKS) or without the fused peak search.
+int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off, int32_t n_events,
+                uint32_t *d_mh, bool peaks, uint32_t threshold, ht_peak *d_out, uint32_t capacity, uint32_t *d_n_found,
+                cudaStream_t st)
+{
+    const ht::Geom &g = ctx->geom;
+    ht::FillArgs a{};
+    a.x = d_x; a.y = d_y; a.z = d_z; a.event_offsets = d_off;
+    a.tth = ctx->d_tth; a.pph = ctx->d_pph;
+    a.g = g;
+    a.rows_per_tile = ctx->rows_per_tile;
+    a.hit_cap = ctx->hit_cap;
+    a.slab_words = ctx->slab_words;
+    a.total_rows = (unsigned long long)n_events * (unsigned long long)g.planes * (unsigned long long)g.n_a;
+    a.mh = d_mh;
+    a.bulk_ok = (g.n_b % 4 == 0) && ((reinterpret_cast<uintptr_t>(d_mh) & 15u) == 0) && env_int("HT_FILL_NO_BULK", 0) == 0;
+    a.threshold = threshold;
+    static_assert(sizeof(ht::PeakOut) == sizeof(ht_peak), "peak record layout");
+    a.out = reinterpret_cast<ht::PeakOut *>(d_out);
+    a.capacity = capacity;
+    a.counters = ctx->d_counters;
+    a.n_found_out = d_n_found;
+    unsigned long long grid = (unsigned long long)ctx->sm_count * (unsigned long long)ctx->fill_ctas_per_sm;
+    // a CTA needs a few rows to work on; tiny problems get fewer CTAs
+    const unsigned long long min_rows = 4;
+    if (grid * min_rows > a.total_rows) grid = (a.total_rows + min_rows - 1) / min_rows;
+    if (grid < 1) grid = 1;
+    if (peaks)
+        ht::fill_stream_kernel<true><<<(unsigned)grid, ht::kFillThreads, ctx->fill_smem, st>>>(a);
+    else
+        ht::fill_stream_kernel<false><<<(unsigned)grid, ht::kFillThreads, ctx->fill_smem, st>>>(a);
+    HT_CUDA(cudaGetLastError());
+    ++ctx->launches;
+    ctx->info[0] = (int32_t)grid; ctx->info[1] = ht::kFillThreads; ctx->info[2] = (int32_t)ctx->fill_smem;
+    ctx->info[3] = ctx->rows_per_tile;
+    return HT_OK;
+}
+
+}  // namespace
+
 int ht_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
             int32_t n_events, int32_t n_hits_total, uint32_t *d_mh, void *cuda_stream)
 {
-    const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh);
+    const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh, true);
     if (rc != HT_OK || n_events == 0) return rc;
     if (!ctx->slab_ok) return HT_ERR_UNSUPPORTED;
+    return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, d_mh, false, 0u, nullptr, 0u, nullptr,
+                       static_cast<cudaStream_t>(cuda_stream));
+}
+
+int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
+                  int32_t n_events, int32_t n_hits_total, uint32_t *d_mh_or_null, uint32_t threshold, ht_peak *d_out,
+                  uint32_t capacity, uint32_t *d_n_found, void *cuda_stream)
+{
+    if (threshold < 1u || !d_n_found || (capacity > 0 && !d_out)) return HT_ERR_INVALID_ARG;
+    const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh_or_null, false);
+    if (rc != HT_OK) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const ht::Geom &g = ctx->geom;
-
-    ht::classify_bucket_kernel<<<n_events, ht::kClassifyThreads, ctx->classify_smem, st>>>(
-        d_x, d_y, d_z, d_event_offsets, ctx->d_tth, ctx->d_pph, g, ctx->d_rec, ctx->d_plane_off);
-    HT_CUDA(cudaGetLastError());
-    ++ctx->launches;
-
-    const long long n_items = (long long)n_events * g.planes * ctx->tiles_per_plane;
-    long long grid = (long long)ctx->sm_count * ctx->fill_ctas_per_sm;
-    if (grid > n_items) grid = n_items;
-    const uint32_t slab_words = (uint32_t)(ctx->slab_bytes / 4u);
-    if (ctx->fill_nbuf == 2)
-        ht::fill_slab_kernel<2><<<(unsigned)grid, ctx->fill_threads, ctx->fill_smem, st>>>(
-            ctx->d_rec, ctx->d_plane_off, g, ctx->rows_per_slab, ctx->tiles_per_plane, n_items, slab_words, d_mh);
-    else
-        ht::fill_slab_kernel<1><<<(unsigned)grid, ctx->fill_threads, ctx->fill_smem, st>>>(
-            ctx->d_rec, ctx->d_plane_off, g, ctx->rows_per_slab, ctx->tiles_per_plane, n_items, slab_words, d_mh);
-    HT_CUDA(cudaGetLastError());
-    ++ctx->launches;
-    ctx->info[0] = (int32_t)grid; ctx->info[1] = ctx->fill_threads; ctx->info[2] = (int32_t)ctx->fill_smem;
-    ctx->info[3] = ctx->rows_per_slab;
-    return HT_OK;
+    if (n_events == 0) {
+        HT_CUDA(cudaMemsetAsync(d_n_found, 0, sizeof(uint32_t), st));
+        return HT_OK;
+    }
+    if (!ctx->slab_ok || (ctx->rows_per_tile < 2 && ctx->geom.n_a > 1)) return HT_ERR_UNSUPPORTED;
+    return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, d_mh_or_null, true, threshold, d_out, capacity,
+                       d_n_found, st);
 }
 
 int ht_fill_naive(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
                   int32_t n_events, int32_t n_hits_total, uint32_t *d_mh, void *cuda_stream)
 {
-    const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh);
+    const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh, true);
     if (rc != HT_OK || n_events == 0) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const ht::Geom &g = ctx->geom;
@@ -358,19 +419,22 @@ int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_t thres
     const unsigned long long total_cells = (unsigned long long)n_events * g.cells;
     const bool vec4 = (g.n_b % 4 == 0) && ((reinterpret_cast<uintptr_t>(d_mh) & 15u) == 0);
     const unsigned long long n_groups = vec4 ? total_cells / 4ull : total_cells;
-    const unsigned long long per_cta = (unsigned long long)ht::kPeaksThreads * ht::kPeaksUnroll;
+    const int U = vec4 ? ctx->peaks_unroll : 4;
+    const unsigned long long per_cta = (unsigned long long)ht::kPeaksThreads * (unsigned long long)U;
     unsigned long long grid = (n_groups + per_cta - 1ull) / per_cta;
-    const unsigned long long cap = (unsigned long long)ctx->sm_count * (unsigned long long)ctx->peaks_ctas_per_sm;
-    if (grid > cap) grid = cap;
+    const unsigned long long resident = (unsigned long long)(vec4 ? ctx->peaks_grid_vec4 : ctx->peaks_grid_vec1);
+    if (grid > resident) grid = resident;
     if (grid < 1ull) grid = 1ull;
     static_assert(sizeof(ht::PeakOut) == sizeof(ht_peak), "peak record layout");
     ht::PeakOut *out = reinterpret_cast<ht::PeakOut *>(d_out);
-    if (vec4)
-        ht::peaks_kernel<4><<<(unsigned)grid, ht::kPeaksThreads, 0, st>>>(d_mh, n_groups, g, threshold, out, capacity,
-                                                                         ctx->d_counters, d_n_found);
-    else
-        ht::peaks_kernel<1><<<(unsigned)grid, ht::kPeaksThreads, 0, st>>>(d_mh, n_groups, g, threshold, out, capacity,
-                                                                         ctx->d_counters, d_n_found);
+#define HT_LAUNCH_PEAKS(V, UU)                                                                                          \
+    ht::peaks_kernel<V, UU><<<(unsigned)grid, ht::kPeaksThreads, 0, st>>>(d_mh, n_groups, g, threshold, out, capacity, \
+                                                                          ctx->d_counters, d_n_found)
+    if (!vec4) HT_LAUNCH_PEAKS(1, 4);
+    else if (U == 2) HT_LAUNCH_PEAKS(4, 2);
+    else if (U == 8) HT_LAUNCH_PEAKS(4, 8);
+    else HT_LAUNCH_PEAKS(4, 4);
+#undef HT_LAUNCH_PEAKS
     HT_CUDA(cudaGetLastError());
     ++ctx->launches;
     ctx->info[4] = (int32_t)grid; ctx->info[5] = ht::kPeaksThreads;
@@ -405,24 +469,27 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
     ht_peak *d_list = reinterpret_cast<ht_peak *>(ctx->d_hres + kResHeader);
     uint32_t found_total = 0u, written = 0u;
     const int slots = ctx->cfg.host_slots;
-    std::vector<int32_t> off_local((size_t)slots + 1);
+    int32_t *off_local = ctx->h_off;      // pinned; reused by the next group only after this group's synchronisation
     for (int e0 = 0; e0 < n_events; e0 += slots) {
         const int ne = (n_events - e0 < slots) ? n_events - e0 : slots;
         const int32_t hb = h_event_offsets[e0];
-        for (int k = 0; k <= ne; ++k) off_local[(size_t)k] = h_event_offsets[e0 + k] - hb;
-        const int32_t nh = off_local[(size_t)ne];
-        // off_local is reused by the next group: the copy below must have consumed it before we overwrite it,
-        // which the synchronisation at the end of this iteration guarantees.
-        HT_CUDA(cudaMemcpyAsync(ctx->d_hoff, off_local.data(), sizeof(int32_t) * (size_t)(ne + 1), cudaMemcpyHostToDevice, st));
-        int rc = ht_fill(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, st);
-        if (rc == HT_ERR_UNSUPPORTED)
-            rc = ht_fill_naive(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, st);
-        if (rc != HT_OK) return rc;
+        for (int k = 0; k <= ne; ++k) off_local[k] = h_event_offsets[e0 + k] - hb;
+        const int32_t nh = off_local[ne];
+        HT_CUDA(cudaMemcpyAsync(ctx->d_hoff, off_local, sizeof(int32_t) * (size_t)(ne + 1), cudaMemcpyHostToDevice, st));
         const uint32_t room = capacity - written;
-        rc = ht_peaks(ctx, ctx->d_hmh, ne, threshold, d_list, room, d_count, st);
+        // the fused kernel (matrix materialised AND peaks found in one pass); shapes it refuses take the two-call path
+        int rc = ht_fill_peaks(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, threshold,
+                               d_list, room, d_count, st);
+        if (rc == HT_ERR_UNSUPPORTED) {
+            rc = ht_fill(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, st);
+            if (rc == HT_ERR_UNSUPPORTED)
+                rc = ht_fill_naive(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, st);
+            if (rc != HT_OK) return rc;
+            rc = ht_peaks(ctx, ctx->d_hmh, ne, threshold, d_list, room, d_count, st);
+        }
         if (rc != HT_OK) return rc;
         // one D2H for count + a first slice of the list; a second one only if the list is longer than the slice
-        const uint32_t slice = room < 4096u ? room : 4096u;
+        const uint32_t slice = room < 1024u ? room : 1024u;
         HT_CUDA(cudaMemcpyAsync(ctx->h_res, ctx->d_hres, kResHeader + sizeof(ht_peak) * (size_t)slice, cudaMemcpyDeviceToHost, st));
         if (h_mh_or_null)
             HT_CUDA(cudaMemcpyAsync(h_mh_or_null + (size_t)e0 * cells, ctx->d_hmh, sizeof(uint32_t) * cells * (size_t)ne,
@@ -463,8 +530,6 @@ void ht_destroy(ht_ctx *ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->cfg.device);
     if (ctx->host_stream) { cudaStreamSynchronize(ctx->host_stream); cudaStreamDestroy(ctx->host_stream); }
-    cudaFree(ctx->d_rec);
-    cudaFree(ctx->d_plane_off);
     cudaFree(ctx->d_tth);
     cudaFree(ctx->d_counters);
     cudaFree(ctx->d_hx);
@@ -472,6 +537,7 @@ void ht_destroy(ht_ctx *ctx)
     cudaFree(ctx->d_hmh);
     cudaFree(ctx->d_hres);
     if (ctx->h_res) cudaFreeHost(ctx->h_res);
+    if (ctx->h_off) cudaFreeHost(ctx->h_off);
     delete ctx;
 }
 
@@ -480,7 +546,7 @@ const char *ht_strerror(int status)
     switch (status) {
     case HT_OK: return "ok";
     case HT_ERR_INVALID_ARG: return "invalid argument";
-    case HT_ERR_UNSUPPORTED: return "binning not supported by the slab kernel (use ht_fill_naive) or call unavailable";
+    case HT_ERR_UNSUPPORTED: return "binning not supported by this kernel (see include/ht.h) or call unavailable";
     case HT_ERR_CUDA: return g_cuda_err;
     case HT_ERR_NOMEM: return "out of memory";
     default: return "unknown status";

@@ -49,17 +49,37 @@ class GpuHough:
         torch.cuda.synchronize()
         return mh
 
-    def peaks(self, mh: torch.Tensor, n_events: int, threshold: int, capacity: int = 1 << 20, stream=None):
+    def fill_peaks(self, batch, threshold: int, capacity: int = 1 << 20, store: bool = True, stream=None):
+        """Fused call.  Returns (mh or None, n_found, peaks)."""
+        dx, dy, dz, doff = self.upload(batch)
+        cells = self.cfg.cells
+        mh = None
+        if store:
+            mh = torch.empty(batch.n_events * cells, dtype=torch.int32, device=self.dev)
+            if mh.numel():
+                mh.fill_(-1)
         out = torch.zeros(max(capacity, 1) * 3, dtype=torch.int32, device=self.dev)
         nf = torch.full((1,), -7, dtype=torch.int32, device=self.dev)
-        B.ht_peaks(self.ctx, mh, n_events, threshold, out if capacity else None, capacity, nf, stream)
+        B.ht_fill_peaks(self.ctx, dx, dy, dz, doff, batch.n_events, batch.n_hits, mh, threshold,
+                        out if capacity else None, capacity, nf, stream)
         torch.cuda.synchronize()
+        return (mh,) + self._peak_result(out, nf, capacity)
+
+    @staticmethod
+    def _peak_result(out, nf, capacity):
         n = int(nf.cpu().numpy().view(np.uint32)[0])
         k = min(n, capacity)
         rec = out[:3 * k].cpu().numpy().view(np.uint32).reshape(k, 3)
         pk = np.empty(k, B.PEAK_DTYPE)
         pk["event"], pk["cell"], pk["count"] = rec[:, 0], rec[:, 1], rec[:, 2]
         return n, pk
+
+    def peaks(self, mh: torch.Tensor, n_events: int, threshold: int, capacity: int = 1 << 20, stream=None):
+        out = torch.zeros(max(capacity, 1) * 3, dtype=torch.int32, device=self.dev)
+        nf = torch.full((1,), -7, dtype=torch.int32, device=self.dev)
+        B.ht_peaks(self.ctx, mh, n_events, threshold, out if capacity else None, capacity, nf, stream)
+        torch.cuda.synchronize()
+        return self._peak_result(out, nf, capacity)
 
 
 def mh_to_numpy(mh: torch.Tensor, bn, n_events: int) -> np.ndarray:

@@ -19,18 +19,34 @@ def _oracle_batch(bn, batch):
     return [oracle_fill(bn, *batch.event(e))[0] for e in range(batch.n_events)]
 
 
-def _check_batch(bn, batch, threshold, naive=False, capacity=1 << 20):
+def _check_batch(bn, batch, threshold, naive=False, capacity=1 << 20, fused=True):
+    """ht_fill (or ht_fill_naive) + ht_peaks, then the fused ht_fill_peaks with and without the matrix store: all three
+    against the oracle, element by element."""
     want_m = _oracle_batch(bn, batch)
+    want_p = oracle_peaks_batch(bn, want_m, threshold)
     with GpuHough(bn, max_events=max(1, batch.n_events), max_hits=batch.n_hits) as g:
         mh = g.fill(batch, naive=naive)
         got = mh_to_numpy(mh, bn, batch.n_events)
         for e in range(batch.n_events):
             np.testing.assert_array_equal(got[e], want_m[e], err_msg=f"event {e}")
         n, pk = g.peaks(mh, batch.n_events, threshold, capacity)
-    want_p = oracle_peaks_batch(bn, want_m, threshold)
-    assert n == len(want_p)
-    if capacity >= n:
-        np.testing.assert_array_equal(sort_peaks(pk, bn.cells), want_p)
+        assert n == len(want_p)
+        if capacity >= n:
+            np.testing.assert_array_equal(sort_peaks(pk, bn.cells), want_p)
+        del mh
+        if fused and not naive:
+            mh2, n2, pk2 = g.fill_peaks(batch, threshold, capacity)
+            got2 = mh_to_numpy(mh2, bn, batch.n_events)
+            for e in range(batch.n_events):
+                np.testing.assert_array_equal(got2[e], want_m[e], err_msg=f"fused, event {e}")
+            assert n2 == len(want_p)
+            if capacity >= n2:
+                np.testing.assert_array_equal(sort_peaks(pk2, bn.cells), want_p)
+            del mh2
+            _, n3, pk3 = g.fill_peaks(batch, threshold, capacity, store=False)
+            assert n3 == len(want_p)
+            if capacity >= n3:
+                np.testing.assert_array_equal(sort_peaks(pk3, bn.cells), want_p)
     return n
 
 
@@ -83,6 +99,11 @@ def test_config5_two_events_sampled():
         got_p = sort_peaks(pk, bn.cells)
         np.testing.assert_array_equal(got_p[got_p["event"] == 1], want_p1)
         assert (got_p["event"] == 0).sum() > 0
+        del mh
+        # the fused kernel without the matrix store must find the same peak set for both events
+        _, n_f, pk_f = g.fill_peaks(batch, wl.threshold, store=False)
+        assert n_f == n
+        np.testing.assert_array_equal(sort_peaks(pk_f, bn.cells), got_p)
 
 
 def test_naive_paper_design_matches_too():
@@ -93,26 +114,57 @@ def test_naive_paper_design_matches_too():
 
 
 # ------------------------------------------------------------------ shapes: ragged tiles, odd sizes, partial ranges
-@pytest.mark.parametrize("dims", [(4, 16, 1000, 1024),      # NA not a multiple of the rows per slab: ragged last tile
+@pytest.mark.parametrize("dims", [(4, 16, 1000, 1024),      # NA not a multiple of the rows per tile: ragged last tile
                                   (3, 5, 77, 36),            # small, odd plane count, NB % 4 == 0
-                                  (1, 1, 1, 4), (2, 2, 5, 8),
-                                  (4, 16, 37, 4096),         # wide rows: few rows per slab
-                                  (2, 3, 300, 12000)])       # one row = 48 KB: one row per slab
-def test_slab_geometries(dims):
+                                  (1, 1, 1, 4), (2, 2, 5, 8), (1, 3, 2, 16), (2, 1, 3, 32),
+                                  (4, 16, 37, 4096),         # wide rows: 3 rows per tile
+                                  (2, 2, 40, 6000),          # 2 rows per tile: the smallest tile the fused scan accepts
+                                  (2, 3, 9, 7), (4, 16, 50, 130), (1, 2, 3, 1),   # NB % 4 != 0: plain stores, scalar scan
+                                  (5, 7, 333, 1001)])
+def test_tile_geometries(dims):
     bn = Binning(*dims)
     batch = generate_batch(1, n_events=2)
     _check_batch(bn, batch, 3)
 
 
-@pytest.mark.parametrize("dims", [(2, 3, 9, 7), (4, 16, 50, 130), (1, 2, 3, 1)])
-def test_shapes_the_slab_kernel_refuses_go_through_the_naive_kernel(dims):
-    bn = Binning(*dims)
+def test_one_row_per_tile_fill_only():
+    """One A row = 48 KB: ht_fill works with 1-row tiles, the fused call refuses (needs 2 rows per tile)."""
+    bn = Binning(2, 3, 300, 12000)
+    batch = generate_batch(1, n_events=2)
+    _check_batch(bn, batch, 3, fused=False)
+    with GpuHough(bn, 2, batch.n_hits) as g:
+        with pytest.raises(B.HtError) as ei:
+            g.fill_peaks(batch, 3)
+        assert ei.value.status == B.HT_ERR_UNSUPPORTED
+
+
+def test_rows_that_do_not_fit_a_tile_go_through_the_naive_kernel():
+    bn = Binning(1, 2, 3, 40000)                            # one row = 160 KB
     batch = generate_batch(1)
     with GpuHough(bn, 1, batch.n_hits) as g:
         with pytest.raises(B.HtError) as ei:
             g.fill(batch)
         assert ei.value.status == B.HT_ERR_UNSUPPORTED
     _check_batch(bn, batch, 2, naive=True)
+
+
+def test_unaligned_matrix_pointer_uses_plain_stores():
+    """d_mh only 4-byte aligned: no bulk stores, same result."""
+    wl = WORKLOADS[1]
+    bn = wl.binning
+    batch = generate_batch(wl, n_events=2)
+    want_m = _oracle_batch(bn, batch)
+    with GpuHough(bn, 2, batch.n_hits) as g:
+        dx, dy, dz, doff = g.upload(batch)
+        buf = torch.full((2 * bn.cells + 4,), -1, dtype=torch.int32, device="cuda")
+        mh = buf[1:1 + 2 * bn.cells]
+        assert mh.data_ptr() % 16 == 4
+        B.ht_fill(g.ctx, dx, dy, dz, doff, 2, batch.n_hits, mh)
+        torch.cuda.synchronize()
+        got = mh_to_numpy(mh, bn, 2)
+        for e in range(2):
+            np.testing.assert_array_equal(got[e], want_m[e])
+        assert int(buf[0]) == -1 and int(buf[-1]) == -1
 
 
 def test_partial_angle_ranges_and_asymmetric_ab_ranges():
@@ -147,7 +199,8 @@ def test_empty_and_degenerate_events():
 
 
 def test_all_hits_in_one_plane_many_hits():
-    # 30000 hits in a narrow cone: one plane gets everything (chunked vote loop, counts far above 255)
+    # 30000 hits in a narrow cone: one plane gets everything (more hits than the shared-memory hit list holds: the list
+    # is rebuilt chunk by chunk for every tile; counts far above 255)
     rng = np.random.default_rng(3)
     n = 30000
     ph = rng.uniform(0.30, 0.35, n); r = rng.uniform(60, 1000, n)
@@ -238,7 +291,7 @@ def test_run_host_end_to_end():
         out2 = np.zeros(3, B.PEAK_DTYPE)
         n2 = B.ht_run_host(g.ctx, batch.x, batch.y, batch.z, batch.event_offsets, 5, batch.n_hits, wl.threshold, out2, 3)
         assert n2 == n
-        assert B.ht_kernel_launches(g.ctx) >= 2 * 3 * 3
+        assert B.ht_kernel_launches(g.ctx) >= 2 * 3            # 2 calls x 3 groups of <= 2 events, one fused kernel each
 
 
 def test_error_codes_on_device_calls():
