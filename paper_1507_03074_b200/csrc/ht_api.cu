@@ -102,9 +102,12 @@ struct ht_ctx {
     // device workspace
     float *d_tth = nullptr, *d_pph = nullptr;
     uint32_t *d_counters = nullptr;
-    // row-stream fill launch geometry
+    // hit buckets written by classify_bucket_kernel (a0): per-hit vote constants grouped by (event, plane)
+    float *d_bx = nullptr, *d_br2 = nullptr, *d_bden = nullptr;
+    int32_t *d_bucket_start = nullptr;     // [max_events * (P+1)]
+    // tile fill launch geometry
     bool slab_ok = false;
-    int rows_per_tile = 0, hit_cap = 0, fill_ctas_per_sm = 0;
+    int rows_slab = 0, fill_ctas_per_sm = 0;
     uint32_t slab_words = 0;
     size_t fill_smem = 0;
     // peak scan launch geometry
@@ -126,7 +129,7 @@ namespace {
 constexpr size_t kResHeader = 16;
 
 struct WorkspaceSizes {
-    size_t tables, counters, host_hits, host_off, host_mh, host_res, total;
+    size_t tables, counters, buckets, bucket_start, host_hits, host_off, host_mh, host_res, total;
 };
 
 WorkspaceSizes workspace_sizes(const ht_config *c)
@@ -136,51 +139,49 @@ WorkspaceSizes workspace_sizes(const ht_config *c)
     const size_t cells = planes * (size_t)c->n_a * (size_t)c->n_b;
     w.tables = align_up(sizeof(float) * (size_t)(c->n_theta + 1 + c->n_phi + 1), 256);
     w.counters = 256;
+    w.buckets = 3 * align_up(sizeof(float) * (size_t)c->max_hits, 256);
+    w.bucket_start = align_up(sizeof(int32_t) * (size_t)c->max_events * (planes + 1), 256);
     if (c->host_slots > 0) {
         w.host_hits = 3 * align_up(sizeof(float) * (size_t)c->max_hits, 256);
         w.host_off = align_up(sizeof(int32_t) * ((size_t)c->max_events + 1), 256);
         w.host_mh = align_up(cells * sizeof(uint32_t) * (size_t)c->host_slots, 256);
         w.host_res = align_up(kResHeader + sizeof(ht_peak) * (size_t)c->host_peak_capacity, 256);
     }
-    w.total = w.tables + w.counters + w.host_hits + w.host_off + w.host_mh + w.host_res;
+    w.total = w.tables + w.counters + w.buckets + w.bucket_start + w.host_hits + w.host_off + w.host_mh + w.host_res;
     return w;
 }
 
-// hit_in_plane() (one interval test per angle) equals the count-of-edges rule of SPEC.md section 2 only for monotone
-// tables; they are monotone for every valid configuration (cot and the pseudo-angle are monotone, rounding keeps that).
-bool tables_monotone(const std::vector<float> &tth, const std::vector<float> &pph)
-{
-    for (size_t k = 1; k < tth.size(); ++k)
-        if (!(tth[k] <= tth[k - 1])) return false;
-    for (size_t k = 1; k < pph.size(); ++k)
-        if (!(pph[k] >= pph[k - 1])) return false;
-    return true;
-}
+// Tile geometry of the fill kernel: a slab of `rows_slab` A rows so that two slabs and the row table of `ctas` CTAs
+// fit the SM's shared memory.  Two CTAs per SM unless that leaves fewer than 4 rows per slab.
+constexpr size_t kClassifySmemMax = 48 * 1024;
 
-// Tile geometry of the row-stream fill: R rows per slab so that two slabs, the hit list and the row table of
-// `ctas_per_sm` CTAs fit the SM's shared memory.
 void plan_fill(ht_ctx *ctx)
 {
     const ht_config &c = ctx->cfg;
     ctx->slab_ok = false;
+    if ((size_t)ctx->geom.planes * sizeof(int) > kClassifySmemMax) return;      // plane counters of the classify kernel
     const size_t row_bytes = (size_t)c.n_b * 4u;
-    const int slab_kb = env_int("HT_FILL_SLAB_KB", 48);
-    int ctas = env_int("HT_FILL_CTAS_PER_SM", 2);
-    int cap = env_int("HT_FILL_HIT_CAP", 1024);
-    if (ctas < 1) ctas = 1;
-    if (ctas > 2) ctas = 2;                                   // __launch_bounds__(kFillThreads, 2)
-    cap = (cap + ht::kFillThreads - 1) / ht::kFillThreads * ht::kFillThreads;
-    if (cap < ht::kFillThreads) cap = ht::kFillThreads;
-    size_t budget = ((size_t)228 * 1024 - (size_t)ctas * 1024) / (size_t)ctas - 256;    // 1 KB per CTA is reserved; 256: static smem
-    if (budget > (size_t)ctx->max_smem_optin) budget = (size_t)ctx->max_smem_optin;
-    const size_t fixed = 12u * (size_t)cap;
-    long long rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
-    if (rows > c.n_a) rows = c.n_a;
-    auto need = [&](long long r) { return 2u * align_up((size_t)r * row_bytes, 16) + fixed + align_up(4u * (size_t)r, 16); };
-    while (rows >= 1 && need(rows) > budget) --rows;
+    const int slab_kb = env_int("HT_FILL_SLAB_KB", 52);
+    const int want_ctas = env_int("HT_FILL_CTAS_PER_SM", 2);
+    auto need = [&](long long r) { return 2u * align_up((size_t)r * row_bytes, 16) + align_up(4u * (size_t)r, 16); };
+    auto rows_for = [&](int ctas) -> long long {
+        size_t budget = ((size_t)228 * 1024 - (size_t)ctas * 1024) / (size_t)ctas - 8192;   // 1 KB/CTA reserved; 8 KB: static smem
+        if (budget > (size_t)ctx->max_smem_optin - 8192) budget = (size_t)ctx->max_smem_optin - 8192;
+        long long rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
+        if (ctas == 1 && rows < 4) rows = 4;
+        if (rows > c.n_a) rows = c.n_a;
+        while (rows >= 1 && need(rows) > budget) --rows;
+        return rows;
+    };
+    int ctas = (want_ctas <= 1) ? 1 : 2;
+    long long rows = rows_for(ctas);
+    if (ctas == 2 && rows < 4 && rows < c.n_a) {
+        const long long r1 = rows_for(1);
+        if (r1 > rows) { rows = r1; ctas = 1; }
+    }
     if (rows < 1) return;                                      // one row does not fit: ht_fill_naive only
-    ctx->rows_per_tile = (int)rows;
-    ctx->hit_cap = cap;
+    if ((long long)c.max_hits * rows >= (1ll << 31)) return;   // the (row, hit) pair index of a tile is an int
+    ctx->rows_slab = (int)rows;
     ctx->slab_words = (uint32_t)(align_up((size_t)rows * row_bytes, 16) / 4u);
     ctx->fill_ctas_per_sm = ctas;
     ctx->fill_smem = need(rows);
@@ -264,6 +265,10 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     if (!dmalloc((void **)&ctx->d_tth, w.tables, "cudaMalloc(tables)")) return fail(rc);
     ctx->d_pph = ctx->d_tth + (cfg->n_theta + 1);
     if (!dmalloc((void **)&ctx->d_counters, w.counters, "cudaMalloc(counters)")) return fail(rc);
+    if (!dmalloc((void **)&ctx->d_bx, w.buckets, "cudaMalloc(hit buckets)")) return fail(rc);
+    ctx->d_br2 = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ctx->d_bx) + w.buckets / 3);
+    ctx->d_bden = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ctx->d_bx) + 2 * (w.buckets / 3));
+    if (!dmalloc((void **)&ctx->d_bucket_start, w.bucket_start, "cudaMalloc(bucket offsets)")) return fail(rc);
     if ((e = cudaMemcpy(ctx->d_tth, tth.data(), tth.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMemcpy(ctx->d_pph, pph.data(), pph.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMemset(ctx->d_counters, 0, w.counters)) != cudaSuccess)
@@ -286,11 +291,10 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     }
 
     plan_fill(ctx);
-    if (ctx->slab_ok && !tables_monotone(tth, pph)) ctx->slab_ok = false;
     if (ctx->slab_ok) {
-        if ((e = cudaFuncSetAttribute(ht::fill_stream_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        if ((e = cudaFuncSetAttribute(ht::fill_tiles_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)ctx->fill_smem)) != cudaSuccess ||
-            (e = cudaFuncSetAttribute(ht::fill_stream_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+            (e = cudaFuncSetAttribute(ht::fill_tiles_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)ctx->fill_smem)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaFuncSetAttribute"));
     }
@@ -319,20 +323,33 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
 
 namespace {
 
-// Launch of the row-stream kernel, with (PEAKS) or without the fused peak search.
+// a0 (classify_bucket_kernel) + the tile kernel, with (PEAKS) or without the fused peak search.
 int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off, int32_t n_events,
                 uint32_t *d_mh, bool peaks, uint32_t threshold, ht_peak *d_out, uint32_t capacity, uint32_t *d_n_found,
                 cudaStream_t st)
 {
     const ht::Geom &g = ctx->geom;
+    ht::classify_bucket_kernel<<<n_events, ht::kClassifyThreads, (size_t)g.planes * sizeof(int), st>>>(
+        d_x, d_y, d_z, d_off, ctx->d_tth, ctx->d_pph, g.n_theta, g.n_phi, ctx->d_bx, ctx->d_br2, ctx->d_bden,
+        ctx->d_bucket_start);
+    HT_CUDA(cudaGetLastError());
+    ++ctx->launches;
+
     ht::FillArgs a{};
-    a.x = d_x; a.y = d_y; a.z = d_z; a.event_offsets = d_off;
-    a.tth = ctx->d_tth; a.pph = ctx->d_pph;
+    a.bx = ctx->d_bx; a.br2 = ctx->d_br2; a.bden = ctx->d_bden; a.bucket_start = ctx->d_bucket_start;
     a.g = g;
-    a.rows_per_tile = ctx->rows_per_tile;
-    a.hit_cap = ctx->hit_cap;
+    // rows stored per tile: the whole slab, minus one halo row on each side for the peak test unless one tile covers a plane
+    int rows_store = ctx->rows_slab < g.n_a ? ctx->rows_slab : g.n_a;
+    a.halo = 0;
+    if (peaks && rows_store < g.n_a) {
+        rows_store = ctx->rows_slab - 2;
+        a.halo = 1;
+    }
+    if (rows_store < 1) return HT_ERR_UNSUPPORTED;
+    a.rows_store = rows_store;
+    a.tiles_per_plane = (g.n_a + rows_store - 1) / rows_store;
     a.slab_words = ctx->slab_words;
-    a.total_rows = (unsigned long long)n_events * (unsigned long long)g.planes * (unsigned long long)g.n_a;
+    a.n_tiles = (unsigned long long)n_events * (unsigned long long)g.planes * (unsigned long long)a.tiles_per_plane;
     a.mh = d_mh;
     a.bulk_ok = (g.n_b % 4 == 0) && ((reinterpret_cast<uintptr_t>(d_mh) & 15u) == 0) && env_int("HT_FILL_NO_BULK", 0) == 0;
     a.threshold = threshold;
@@ -342,18 +359,16 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.counters = ctx->d_counters;
     a.n_found_out = d_n_found;
     unsigned long long grid = (unsigned long long)ctx->sm_count * (unsigned long long)ctx->fill_ctas_per_sm;
-    // a CTA needs a few rows to work on; tiny problems get fewer CTAs
-    const unsigned long long min_rows = 4;
-    if (grid * min_rows > a.total_rows) grid = (a.total_rows + min_rows - 1) / min_rows;
+    if (grid > a.n_tiles) grid = a.n_tiles;
     if (grid < 1) grid = 1;
     if (peaks)
-        ht::fill_stream_kernel<true><<<(unsigned)grid, ht::kFillThreads, ctx->fill_smem, st>>>(a);
+        ht::fill_tiles_kernel<true><<<(unsigned)grid, ht::kFillThreads, ctx->fill_smem, st>>>(a);
     else
-        ht::fill_stream_kernel<false><<<(unsigned)grid, ht::kFillThreads, ctx->fill_smem, st>>>(a);
+        ht::fill_tiles_kernel<false><<<(unsigned)grid, ht::kFillThreads, ctx->fill_smem, st>>>(a);
     HT_CUDA(cudaGetLastError());
     ++ctx->launches;
     ctx->info[0] = (int32_t)grid; ctx->info[1] = ht::kFillThreads; ctx->info[2] = (int32_t)ctx->fill_smem;
-    ctx->info[3] = ctx->rows_per_tile;
+    ctx->info[3] = rows_store;
     return HT_OK;
 }
 
@@ -381,7 +396,7 @@ int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const float *
         HT_CUDA(cudaMemsetAsync(d_n_found, 0, sizeof(uint32_t), st));
         return HT_OK;
     }
-    if (!ctx->slab_ok || (ctx->rows_per_tile < 2 && ctx->geom.n_a > 1)) return HT_ERR_UNSUPPORTED;
+    if (!ctx->slab_ok || (ctx->rows_slab < 3 && ctx->rows_slab < ctx->geom.n_a)) return HT_ERR_UNSUPPORTED;
     return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, d_mh_or_null, true, threshold, d_out, capacity,
                        d_n_found, st);
 }
@@ -532,6 +547,8 @@ void ht_destroy(ht_ctx *ctx)
     if (ctx->host_stream) { cudaStreamSynchronize(ctx->host_stream); cudaStreamDestroy(ctx->host_stream); }
     cudaFree(ctx->d_tth);
     cudaFree(ctx->d_counters);
+    cudaFree(ctx->d_bx);
+    cudaFree(ctx->d_bucket_start);
     cudaFree(ctx->d_hx);
     cudaFree(ctx->d_hoff);
     cudaFree(ctx->d_hmh);
