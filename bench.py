@@ -293,11 +293,11 @@ def bench_ours(args):
         kernels, kernel_ms = {}, {}
         if "fused" in res:
             f = res["fused"][1][0]
-            kernels["ht_fill_peaks"] = roof("fill_stream_kernel<true> (ht_fill_peaks: classify+vote+store+peak test+compaction)",
+            kernels["ht_fill_peaks"] = roof("classify_bucket_kernel + fill_tiles_kernel<true> (ht_fill_peaks: classify, vote, store, peak test, compaction)",
                                             m_bytes + hit_bytes + pk_bytes, mean(f))
             kernel_ms.update(fused_median=statistics.median(f), fused_mean=mean(f), fused_step_mean=res["fused"][0])
         sp_fill, sp_peaks = res["split"][1]
-        kernels["ht_fill"] = roof("fill_stream_kernel<false> (ht_fill: classify+vote+store)", m_bytes + hit_bytes, mean(sp_fill))
+        kernels["ht_fill"] = roof("classify_bucket_kernel + fill_tiles_kernel<false> (ht_fill: classify, vote, store)", m_bytes + hit_bytes, mean(sp_fill))
         kernels["ht_peaks"] = roof("peaks_kernel (ht_peaks: scan+compaction)", m_bytes + pk_bytes, mean(sp_peaks))
         kernel_ms.update(fill_median=statistics.median(sp_fill), fill_mean=mean(sp_fill),
                          peaks_median=statistics.median(sp_peaks), peaks_mean=mean(sp_peaks),

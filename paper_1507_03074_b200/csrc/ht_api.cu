@@ -102,14 +102,15 @@ struct ht_ctx {
     // device workspace
     float *d_tth = nullptr, *d_pph = nullptr;
     uint32_t *d_counters = nullptr;
-    // hit buckets written by classify_bucket_kernel (a0): per-hit vote constants grouped by (event, plane)
+    // hit buckets written by the fill kernel's prologue (a0): per-hit vote constants grouped by (event, plane)
     float *d_bx = nullptr, *d_br2 = nullptr, *d_bden = nullptr;
+    int32_t *d_hplane = nullptr, *d_hrel = nullptr;   // [max_hits] phase-1 spill
     int32_t *d_bucket_start = nullptr;     // [max_events * (P+1)]
-    // tile fill launch geometry
-    bool slab_ok = false;
-    int rows_slab = 0, fill_ctas_per_sm = 0;
-    uint32_t slab_words = 0;
-    size_t fill_smem = 0;
+    uint32_t *d_counts = nullptr;          // [max_events * P], zero between calls
+    // tile fill launch geometry: per-kernel dynamic shared memory budget ([0]: ht_fill, [1]: fused peaks), and whether
+    // the device can run the kernel at all (one CTA of 1024 threads per SM, cooperative launch for mode 0)
+    bool fill_ok = false;
+    size_t fill_smem_max[2] = {0, 0};
     // peak scan launch geometry
     int peaks_unroll = 4, peaks_grid_vec4 = 0, peaks_grid_vec1 = 0;
     // host path (ht_run_host)
@@ -129,7 +130,7 @@ namespace {
 constexpr size_t kResHeader = 16;
 
 struct WorkspaceSizes {
-    size_t tables, counters, buckets, bucket_start, host_hits, host_off, host_mh, host_res, total;
+    size_t tables, counters, buckets, bucket_start, counts, host_hits, host_off, host_mh, host_res, total;
 };
 
 WorkspaceSizes workspace_sizes(const ht_config *c)
@@ -139,53 +140,35 @@ WorkspaceSizes workspace_sizes(const ht_config *c)
     const size_t cells = planes * (size_t)c->n_a * (size_t)c->n_b;
     w.tables = align_up(sizeof(float) * (size_t)(c->n_theta + 1 + c->n_phi + 1), 256);
     w.counters = 256;
-    w.buckets = 3 * align_up(sizeof(float) * (size_t)c->max_hits, 256);
+    w.buckets = 5 * align_up(sizeof(float) * (size_t)c->max_hits, 256);      // bx, br2, bden, h_plane, h_rel
     w.bucket_start = align_up(sizeof(int32_t) * (size_t)c->max_events * (planes + 1), 256);
+    w.counts = align_up(sizeof(uint32_t) * (size_t)c->max_events * planes, 256);
     if (c->host_slots > 0) {
         w.host_hits = 3 * align_up(sizeof(float) * (size_t)c->max_hits, 256);
         w.host_off = align_up(sizeof(int32_t) * ((size_t)c->max_events + 1), 256);
         w.host_mh = align_up(cells * sizeof(uint32_t) * (size_t)c->host_slots, 256);
         w.host_res = align_up(kResHeader + sizeof(ht_peak) * (size_t)c->host_peak_capacity, 256);
     }
-    w.total = w.tables + w.counters + w.buckets + w.bucket_start + w.host_hits + w.host_off + w.host_mh + w.host_res;
+    w.total = w.tables + w.counters + w.buckets + w.bucket_start + w.counts + w.host_hits + w.host_off + w.host_mh + w.host_res;
     return w;
 }
 
-// Tile geometry of the fill kernel: a slab of `rows_slab` A rows so that two slabs and the row table of `ctas` CTAs
-// fit the SM's shared memory.  Two CTAs per SM unless that leaves fewer than 4 rows per slab.
-constexpr size_t kClassifySmemMax = 48 * 1024;
+// Tile geometry of the fill kernel for one call: the largest slab (rows of NB cells) such that four slabs (two per warp
+// group), the row tables, and -- in mode 1 -- the plane offsets and the uint16 hit index fit the CTA's shared memory.
+struct FillPlan {
+    bool ok = false;
+    int mode = 0, groups = 2, rows_slab = 0;
+    uint32_t slab_words = 0;
+    size_t smem = 0;
+};
 
-void plan_fill(ht_ctx *ctx)
+size_t fill_smem_bytes(const ht_config &c, long long rows, int mode, long long n_hits, int groups)
 {
-    const ht_config &c = ctx->cfg;
-    ctx->slab_ok = false;
-    if ((size_t)ctx->geom.planes * sizeof(int) > kClassifySmemMax) return;      // plane counters of the classify kernel
-    const size_t row_bytes = (size_t)c.n_b * 4u;
-    const int slab_kb = env_int("HT_FILL_SLAB_KB", 52);
-    const int want_ctas = env_int("HT_FILL_CTAS_PER_SM", 2);
-    auto need = [&](long long r) { return 2u * align_up((size_t)r * row_bytes, 16) + align_up(4u * (size_t)r, 16); };
-    auto rows_for = [&](int ctas) -> long long {
-        size_t budget = ((size_t)228 * 1024 - (size_t)ctas * 1024) / (size_t)ctas - 8192;   // 1 KB/CTA reserved; 8 KB: static smem
-        if (budget > (size_t)ctx->max_smem_optin - 8192) budget = (size_t)ctx->max_smem_optin - 8192;
-        long long rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
-        if (ctas == 1 && rows < 4) rows = 4;
-        if (rows > c.n_a) rows = c.n_a;
-        while (rows >= 1 && need(rows) > budget) --rows;
-        return rows;
-    };
-    int ctas = (want_ctas <= 1) ? 1 : 2;
-    long long rows = rows_for(ctas);
-    if (ctas == 2 && rows < 4 && rows < c.n_a) {
-        const long long r1 = rows_for(1);
-        if (r1 > rows) { rows = r1; ctas = 1; }
-    }
-    if (rows < 1) return;                                      // one row does not fit: ht_fill_naive only
-    if ((long long)c.max_hits * rows >= (1ll << 31)) return;   // the (row, hit) pair index of a tile is an int
-    ctx->rows_slab = (int)rows;
-    ctx->slab_words = (uint32_t)(align_up((size_t)rows * row_bytes, 16) / 4u);
-    ctx->fill_ctas_per_sm = ctas;
-    ctx->fill_smem = need(rows);
-    ctx->slab_ok = true;
+    const size_t slab = align_up((size_t)rows * (size_t)c.n_b * 4u, 16);
+    size_t b = 2u * (size_t)groups * slab + 2u * 4u * 4u * (size_t)(rows + 4);     // slabs, two_a[2 groups][4 ring entries][rows + 4]
+    b += 4u * ((size_t)c.n_theta * (size_t)c.n_phi + 1u);
+    if (mode == 1) b += 2u * (size_t)n_hits;
+    return align_up(b, 16);
 }
 
 int check_fill_args(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off,
@@ -266,9 +249,17 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     ctx->d_pph = ctx->d_tth + (cfg->n_theta + 1);
     if (!dmalloc((void **)&ctx->d_counters, w.counters, "cudaMalloc(counters)")) return fail(rc);
     if (!dmalloc((void **)&ctx->d_bx, w.buckets, "cudaMalloc(hit buckets)")) return fail(rc);
-    ctx->d_br2 = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ctx->d_bx) + w.buckets / 3);
-    ctx->d_bden = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ctx->d_bx) + 2 * (w.buckets / 3));
+    {
+        unsigned char *b0 = reinterpret_cast<unsigned char *>(ctx->d_bx);
+        const size_t one = w.buckets / 5;
+        ctx->d_br2 = reinterpret_cast<float *>(b0 + one);
+        ctx->d_bden = reinterpret_cast<float *>(b0 + 2 * one);
+        ctx->d_hplane = reinterpret_cast<int32_t *>(b0 + 3 * one);
+        ctx->d_hrel = reinterpret_cast<int32_t *>(b0 + 4 * one);
+    }
     if (!dmalloc((void **)&ctx->d_bucket_start, w.bucket_start, "cudaMalloc(bucket offsets)")) return fail(rc);
+    if (!dmalloc((void **)&ctx->d_counts, w.counts, "cudaMalloc(bucket counts)")) return fail(rc);
+    if ((e = cudaMemset(ctx->d_counts, 0, w.counts)) != cudaSuccess) return fail(cuda_fail(e, "cudaMemset(bucket counts)"));
     if ((e = cudaMemcpy(ctx->d_tth, tth.data(), tth.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMemcpy(ctx->d_pph, pph.data(), pph.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMemset(ctx->d_counters, 0, w.counters)) != cudaSuccess)
@@ -290,13 +281,28 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
             return fail(cuda_fail(e, "cudaStreamCreate"));
     }
 
-    plan_fill(ctx);
-    if (ctx->slab_ok) {
+    {   // fill kernel: one CTA per SM with as much dynamic shared memory as the device gives
+        cudaFuncAttributes fa0{}, fa1{};
+        int coop = 0;
+        if ((e = cudaFuncGetAttributes(&fa0, ht::fill_tiles_kernel<false>)) != cudaSuccess ||
+            (e = cudaFuncGetAttributes(&fa1, ht::fill_tiles_kernel<true>)) != cudaSuccess ||
+            (e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, cfg->device)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaFuncGetAttributes(fill kernel)"));
+        const size_t optin = (size_t)ctx->max_smem_optin;
+        ctx->fill_smem_max[0] = optin > fa0.sharedSizeBytes ? optin - fa0.sharedSizeBytes : 0;
+        ctx->fill_smem_max[1] = optin > fa1.sharedSizeBytes ? optin - fa1.sharedSizeBytes : 0;
         if ((e = cudaFuncSetAttribute(ht::fill_tiles_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)ctx->fill_smem)) != cudaSuccess ||
+                                      (int)ctx->fill_smem_max[0])) != cudaSuccess ||
             (e = cudaFuncSetAttribute(ht::fill_tiles_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)ctx->fill_smem)) != cudaSuccess)
+                                      (int)ctx->fill_smem_max[1])) != cudaSuccess)
             return fail(cuda_fail(e, "cudaFuncSetAttribute"));
+        int occ0 = 0, occ1 = 0;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ0, ht::fill_tiles_kernel<false>, ht::kFillThreads,
+                                                               ctx->fill_smem_max[0])) != cudaSuccess ||
+            (e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, ht::fill_tiles_kernel<true>, ht::kFillThreads,
+                                                               ctx->fill_smem_max[1])) != cudaSuccess)
+            return fail(cuda_fail(e, "fill kernel occupancy"));
+        ctx->fill_ok = coop && occ0 >= 1 && occ1 >= 1;
     }
     // peak scan: a persistent grid of exactly the CTAs that are resident at once (a grid-stride loop over more CTAs
     // than fit would run the excess as a second, partly empty wave)
@@ -323,33 +329,88 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
 
 namespace {
 
-// a0 (classify_bucket_kernel) + the tile kernel, with (PEAKS) or without the fused peak search.
+FillPlan plan_fill(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool peaks)
+{
+    FillPlan pl;
+    if (!ctx->fill_ok) return pl;
+    const ht_config &c = ctx->cfg;
+    const size_t budget = ctx->fill_smem_max[peaks ? 1 : 0];
+    const size_t row_bytes = (size_t)c.n_b * 4u;
+    const long long planes = (long long)c.n_theta * c.n_phi;
+    // mode 1 (per-CTA shared-memory hit index): one event, uint16 indices and plane ids, an index of at most 48 KB
+    const int force = env_int("HT_FILL_MODE", -1);
+    int mode = (n_events == 1 && n_hits <= 24576 && planes < 65535) ? 1 : 0;
+    if (force == 0) mode = 0;
+    const int slab_kb = env_int("HT_FILL_SLAB_KB", 0);
+    auto rows_for = [&](int md, int groups) -> long long {
+        long long rows = c.n_a;
+        if (slab_kb > 0 && rows > (long long)((size_t)slab_kb * 1024u / row_bytes)) rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
+        if (rows < 1) rows = 1;
+        if (fill_smem_bytes(c, rows, md, n_hits, groups) > budget) {          // largest rows that fit (bisection)
+            long long lo = 0, hi = rows;
+            while (hi - lo > 1) {
+                const long long mid = (lo + hi) / 2;
+                if (fill_smem_bytes(c, mid, md, n_hits, groups) <= budget) lo = mid; else hi = mid;
+            }
+            rows = lo;
+        }
+        // mode 1 sorts in the slab space: plane id + slot, 4 bytes per hit
+        if (md == 1 && 4u * (size_t)n_hits > 2u * (size_t)groups * align_up((size_t)rows * row_bytes, 16)) return 0;
+        return rows;
+    };
+    for (;; mode = 0) {
+        int groups = env_int("HT_FILL_GROUPS", 2) == 1 ? 1 : 2;
+        long long rows = rows_for(mode, groups);
+        if (groups == 2 && rows < 4 && rows < c.n_a) {                        // wide rows: one pipeline with two big slabs
+            const long long r1 = rows_for(mode, 1);
+            if (r1 > rows) { rows = r1; groups = 1; }
+        }
+        if (rows >= 1) {
+            pl.ok = true;
+            pl.mode = mode;
+            pl.groups = groups;
+            pl.rows_slab = (int)rows;
+            pl.slab_words = (uint32_t)(align_up((size_t)rows * row_bytes, 16) / 4u);
+            pl.smem = fill_smem_bytes(c, rows, mode, n_hits, groups);
+            return pl;
+        }
+        if (mode == 0) return pl;                                              // one row does not fit: ht_fill_naive only
+    }
+}
+
+// The fill kernel (prologue a0 + tiles a1-a3), with (PEAKS: + a4-a5) or without the fused peak search.
 int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off, int32_t n_events,
-                uint32_t *d_mh, bool peaks, uint32_t threshold, ht_peak *d_out, uint32_t capacity, uint32_t *d_n_found,
-                cudaStream_t st)
+                int32_t n_hits_total, uint32_t *d_mh, bool peaks, uint32_t threshold, ht_peak *d_out, uint32_t capacity,
+                uint32_t *d_n_found, cudaStream_t st)
 {
     const ht::Geom &g = ctx->geom;
-    ht::classify_bucket_kernel<<<n_events, ht::kClassifyThreads, (size_t)g.planes * sizeof(int), st>>>(
-        d_x, d_y, d_z, d_off, ctx->d_tth, ctx->d_pph, g.n_theta, g.n_phi, ctx->d_bx, ctx->d_br2, ctx->d_bden,
-        ctx->d_bucket_start);
-    HT_CUDA(cudaGetLastError());
-    ++ctx->launches;
-
+    const FillPlan pl = plan_fill(ctx, n_events, n_hits_total, peaks);
+    if (!pl.ok) return HT_ERR_UNSUPPORTED;
     ht::FillArgs a{};
-    a.bx = ctx->d_bx; a.br2 = ctx->d_br2; a.bden = ctx->d_bden; a.bucket_start = ctx->d_bucket_start;
+    a.x = d_x; a.y = d_y; a.z = d_z; a.event_offsets = d_off; a.n_events = n_events; a.n_hits = n_hits_total;
+    a.tth = ctx->d_tth; a.pph = ctx->d_pph;
+    a.mode = pl.mode;
+    a.groups = pl.groups;
+    a.counts = ctx->d_counts; a.bucket_start = ctx->d_bucket_start; a.h_plane = ctx->d_hplane; a.h_rel = ctx->d_hrel;
+    a.bx = ctx->d_bx; a.br2 = ctx->d_br2; a.bden = ctx->d_bden;
+    a.bar = ctx->d_counters + 2;
     a.g = g;
+    a.rows_slab = pl.rows_slab;
     // rows stored per tile: the whole slab, minus one halo row on each side for the peak test unless one tile covers a plane
-    int rows_store = ctx->rows_slab < g.n_a ? ctx->rows_slab : g.n_a;
+    int rows_store = pl.rows_slab < g.n_a ? pl.rows_slab : g.n_a;
     a.halo = 0;
     if (peaks && rows_store < g.n_a) {
-        rows_store = ctx->rows_slab - 2;
+        rows_store = pl.rows_slab - 2;
         a.halo = 1;
     }
     if (rows_store < 1) return HT_ERR_UNSUPPORTED;
     a.rows_store = rows_store;
     a.tiles_per_plane = (g.n_a + rows_store - 1) / rows_store;
-    a.slab_words = ctx->slab_words;
-    a.n_tiles = (unsigned long long)n_events * (unsigned long long)g.planes * (unsigned long long)a.tiles_per_plane;
+    a.slab_words = pl.slab_words;
+    const unsigned long long n_tiles =
+        (unsigned long long)n_events * (unsigned long long)g.planes * (unsigned long long)a.tiles_per_plane;
+    if (n_tiles >= (1ull << 31)) return HT_ERR_UNSUPPORTED;        // tile indices are 32-bit in the kernel
+    a.n_tiles = (uint32_t)n_tiles;
     a.mh = d_mh;
     a.bulk_ok = (g.n_b % 4 == 0) && ((reinterpret_cast<uintptr_t>(d_mh) & 15u) == 0) && env_int("HT_FILL_NO_BULK", 0) == 0;
     a.threshold = threshold;
@@ -358,17 +419,29 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.capacity = capacity;
     a.counters = ctx->d_counters;
     a.n_found_out = d_n_found;
-    unsigned long long grid = (unsigned long long)ctx->sm_count * (unsigned long long)ctx->fill_ctas_per_sm;
-    if (grid > a.n_tiles) grid = a.n_tiles;
+    // one CTA per SM, `groups` tile pipelines (warp groups) per CTA: V = groups * grid virtual CTAs
+    const unsigned long long ng = (unsigned long long)pl.groups;
+    unsigned long long grid = (unsigned long long)ctx->sm_count;
+    if (grid > (n_tiles + ng - 1ull) / ng) grid = (n_tiles + ng - 1ull) / ng;
     if (grid < 1) grid = 1;
-    if (peaks)
-        ht::fill_tiles_kernel<true><<<(unsigned)grid, ht::kFillThreads, ctx->fill_smem, st>>>(a);
-    else
-        ht::fill_tiles_kernel<false><<<(unsigned)grid, ht::kFillThreads, ctx->fill_smem, st>>>(a);
-    HT_CUDA(cudaGetLastError());
+    const unsigned long long V = ng * grid;
+    const unsigned long long dep = V / (unsigned long long)a.tiles_per_plane;
+    a.dk = (int)(V % (unsigned long long)a.tiles_per_plane);
+    a.dpl = (int)(dep % (unsigned long long)g.planes);
+    a.dev = (int)(dep / (unsigned long long)g.planes);
+    if (pl.mode == 0) {     // the prologue synchronises the grid: co-residency guaranteed by a cooperative launch
+        void *params[] = {&a};
+        const void *fn = peaks ? reinterpret_cast<const void *>(ht::fill_tiles_kernel<true>)
+                               : reinterpret_cast<const void *>(ht::fill_tiles_kernel<false>);
+        HT_CUDA(cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(ht::kFillThreads), params, pl.smem, st));
+    } else {
+        if (peaks) ht::fill_tiles_kernel<true><<<(unsigned)grid, ht::kFillThreads, pl.smem, st>>>(a);
+        else ht::fill_tiles_kernel<false><<<(unsigned)grid, ht::kFillThreads, pl.smem, st>>>(a);
+        HT_CUDA(cudaGetLastError());
+    }
     ++ctx->launches;
-    ctx->info[0] = (int32_t)grid; ctx->info[1] = ht::kFillThreads; ctx->info[2] = (int32_t)ctx->fill_smem;
-    ctx->info[3] = rows_store;
+    ctx->info[0] = (int32_t)grid; ctx->info[1] = ht::kFillThreads; ctx->info[2] = (int32_t)pl.smem;
+    ctx->info[3] = rows_store; ctx->info[7] = pl.mode;
     return HT_OK;
 }
 
@@ -379,8 +452,7 @@ int ht_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, c
 {
     const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh, true);
     if (rc != HT_OK || n_events == 0) return rc;
-    if (!ctx->slab_ok) return HT_ERR_UNSUPPORTED;
-    return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, d_mh, false, 0u, nullptr, 0u, nullptr,
+    return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh, false, 0u, nullptr, 0u, nullptr,
                        static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -396,8 +468,7 @@ int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const float *
         HT_CUDA(cudaMemsetAsync(d_n_found, 0, sizeof(uint32_t), st));
         return HT_OK;
     }
-    if (!ctx->slab_ok || (ctx->rows_slab < 3 && ctx->rows_slab < ctx->geom.n_a)) return HT_ERR_UNSUPPORTED;
-    return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, d_mh_or_null, true, threshold, d_out, capacity,
+    return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh_or_null, true, threshold, d_out, capacity,
                        d_n_found, st);
 }
 
@@ -549,6 +620,7 @@ void ht_destroy(ht_ctx *ctx)
     cudaFree(ctx->d_counters);
     cudaFree(ctx->d_bx);
     cudaFree(ctx->d_bucket_start);
+    cudaFree(ctx->d_counts);
     cudaFree(ctx->d_hx);
     cudaFree(ctx->d_hoff);
     cudaFree(ctx->d_hmh);
