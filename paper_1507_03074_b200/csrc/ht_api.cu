@@ -354,8 +354,9 @@ FillPlan plan_fill(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool pea
             }
             rows = lo;
         }
-        // mode 1 sorts in the slab space: plane id + slot, 4 bytes per hit
-        if (md == 1 && 4u * (size_t)n_hits > 2u * (size_t)groups * align_up((size_t)rows * row_bytes, 16)) return 0;
+        // mode 1 sorts in the slab space: plane id + slot, 4 bytes per hit, and a copy of the angle tables
+        if (md == 1 && 4u * (size_t)n_hits + 4u * (size_t)(c.n_theta + c.n_phi + 4) >
+                           2u * (size_t)groups * align_up((size_t)rows * row_bytes, 16)) return 0;
         return rows;
     };
     for (;; mode = 0) {
