@@ -157,16 +157,16 @@ WorkspaceSizes workspace_sizes(const ht_config *c)
 // group), the row tables, and -- in mode 1 -- the plane offsets and the uint16 hit index fit the CTA's shared memory.
 struct FillPlan {
     bool ok = false;
-    int mode = 0, groups = 2, rows_slab = 0;
+    int mode = 0, rows_slab = 0, hit_cap = 0;
     uint32_t slab_words = 0;
     size_t smem = 0;
 };
 
-size_t fill_smem_bytes(const ht_config &c, long long rows, int mode, long long n_hits, int groups)
+size_t fill_smem_bytes(const ht_config &c, long long rows, int mode, long long n_hits)
 {
     const size_t slab = align_up((size_t)rows * (size_t)c.n_b * 4u, 16);
-    size_t b = 2u * (size_t)groups * slab + 2u * 4u * 4u * (size_t)(rows + 4);     // slabs, two_a[2 groups][4 ring entries][rows + 4]
-    b += 4u * ((size_t)c.n_theta * (size_t)c.n_phi + 1u);
+    size_t b = 2u * slab + 4u * 4u * (size_t)(rows + 4);     // two slabs, two_a[4 ring entries][rows + 4]
+    b += align_up(4u * ((size_t)c.n_theta * (size_t)c.n_phi + 1u), 16);      // plane offsets, padded: the staged hits are float4
     if (mode == 1) b += 2u * (size_t)n_hits;
     return align_up(b, 16);
 }
@@ -342,37 +342,37 @@ FillPlan plan_fill(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool pea
     int mode = (n_events == 1 && n_hits <= 24576 && planes < 65535) ? 1 : 0;
     if (force == 0) mode = 0;
     const int slab_kb = env_int("HT_FILL_SLAB_KB", 0);
-    auto rows_for = [&](int md, int groups) -> long long {
+    auto rows_for = [&](int md) -> long long {
         long long rows = c.n_a;
         if (slab_kb > 0 && rows > (long long)((size_t)slab_kb * 1024u / row_bytes)) rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
         if (rows < 1) rows = 1;
-        if (fill_smem_bytes(c, rows, md, n_hits, groups) > budget) {          // largest rows that fit (bisection)
+        if (fill_smem_bytes(c, rows, md, n_hits) > budget) {                  // largest rows that fit (bisection)
             long long lo = 0, hi = rows;
             while (hi - lo > 1) {
                 const long long mid = (lo + hi) / 2;
-                if (fill_smem_bytes(c, mid, md, n_hits, groups) <= budget) lo = mid; else hi = mid;
+                if (fill_smem_bytes(c, mid, md, n_hits) <= budget) lo = mid; else hi = mid;
             }
             rows = lo;
         }
         // mode 1 sorts in the slab space: plane id + slot, 4 bytes per hit, and a copy of the angle tables
         if (md == 1 && 4u * (size_t)n_hits + 4u * (size_t)(c.n_theta + c.n_phi + 4) >
-                           2u * (size_t)groups * align_up((size_t)rows * row_bytes, 16)) return 0;
+                           2u * align_up((size_t)rows * row_bytes, 16)) return 0;
         return rows;
     };
     for (;; mode = 0) {
-        int groups = env_int("HT_FILL_GROUPS", 2) == 1 ? 1 : 2;
-        long long rows = rows_for(mode, groups);
-        if (groups == 2 && rows < 4 && rows < c.n_a) {                        // wide rows: one pipeline with two big slabs
-            const long long r1 = rows_for(mode, 1);
-            if (r1 > rows) { rows = r1; groups = 1; }
-        }
+        const long long rows = rows_for(mode);
         if (rows >= 1) {
             pl.ok = true;
             pl.mode = mode;
-            pl.groups = groups;
             pl.rows_slab = (int)rows;
             pl.slab_words = (uint32_t)(align_up((size_t)rows * row_bytes, 16) / 4u);
-            pl.smem = fill_smem_bytes(c, rows, mode, n_hits, groups);
+            pl.smem = fill_smem_bytes(c, rows, mode, n_hits);
+            // what is left of the budget stages the hits of two tiles (x, r2, den, rc: 16 bytes per hit), up to 512 per tile
+            long long cap = ((long long)(budget - pl.smem) / 32) / 32 * 32;
+            if (cap > 512) cap = 512;
+            if (env_int("HT_FILL_HIT_CAP", -1) >= 0 && cap > env_int("HT_FILL_HIT_CAP", -1)) cap = env_int("HT_FILL_HIT_CAP", -1) / 32 * 32;
+            pl.hit_cap = (int)cap;
+            pl.smem += (size_t)cap * 32u;
             return pl;
         }
         if (mode == 0) return pl;                                              // one row does not fit: ht_fill_naive only
@@ -391,7 +391,7 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.x = d_x; a.y = d_y; a.z = d_z; a.event_offsets = d_off; a.n_events = n_events; a.n_hits = n_hits_total;
     a.tth = ctx->d_tth; a.pph = ctx->d_pph;
     a.mode = pl.mode;
-    a.groups = pl.groups;
+    a.hit_cap = pl.hit_cap;
     a.counts = ctx->d_counts; a.bucket_start = ctx->d_bucket_start; a.h_plane = ctx->d_hplane; a.h_rel = ctx->d_hrel;
     a.bx = ctx->d_bx; a.br2 = ctx->d_br2; a.bden = ctx->d_bden;
     a.bar = ctx->d_counters + 2;
@@ -420,12 +420,11 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.capacity = capacity;
     a.counters = ctx->d_counters;
     a.n_found_out = d_n_found;
-    // one CTA per SM, `groups` tile pipelines (warp groups) per CTA: V = groups * grid virtual CTAs
-    const unsigned long long ng = (unsigned long long)pl.groups;
+    // one CTA per SM; CTA c takes tiles c, c + grid, ...
     unsigned long long grid = (unsigned long long)ctx->sm_count;
-    if (grid > (n_tiles + ng - 1ull) / ng) grid = (n_tiles + ng - 1ull) / ng;
+    if (grid > n_tiles) grid = n_tiles;
     if (grid < 1) grid = 1;
-    const unsigned long long V = ng * grid;
+    const unsigned long long V = grid;
     const unsigned long long dep = V / (unsigned long long)a.tiles_per_plane;
     a.dk = (int)(V % (unsigned long long)a.tiles_per_plane);
     a.dpl = (int)(dep % (unsigned long long)g.planes);
