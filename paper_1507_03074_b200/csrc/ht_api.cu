@@ -109,6 +109,7 @@ struct ht_ctx {
     uint32_t *d_counts = nullptr;          // [max_events * P], zero between calls
     // tile fill launch geometry: per-kernel dynamic shared memory budget ([0]: ht_fill, [1]: fused peaks), and whether
     // the device can run the kernel at all (one CTA of 1024 threads per SM, cooperative launch for mode 0)
+    uint32_t bar_epoch = 0, tile_epoch = 0;   // host mirrors of the two device counters that only grow (d_counters[4], [5])
     bool fill_ok = false;
     size_t fill_smem_max[2] = {0, 0};
     // peak scan launch geometry
@@ -341,7 +342,9 @@ FillPlan plan_fill(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool pea
     const int force = env_int("HT_FILL_MODE", -1);
     int mode = (n_events == 1 && n_hits <= 24576 && planes < 65535) ? 1 : 0;
     if (force == 0) mode = 0;
-    const int slab_kb = env_int("HT_FILL_SLAB_KB", 0);
+    // without the fused peak search the kernel is purely store-bound and measured fastest with slabs of <= 96 KB
+    // (config 2, B200: 51.5 us at 96 KB, 53.4 at 100 KB, 59.4 at 104 KB); with it, the largest slab wins (fewer halo rows)
+    const int slab_kb = env_int("HT_FILL_SLAB_KB", peaks ? 0 : 96);
     auto rows_for = [&](int md) -> long long {
         long long rows = c.n_a;
         if (slab_kb > 0 && rows > (long long)((size_t)slab_kb * 1024u / row_bytes)) rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
@@ -424,21 +427,21 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     unsigned long long grid = (unsigned long long)ctx->sm_count;
     if (grid > n_tiles) grid = n_tiles;
     if (grid < 1) grid = 1;
-    const unsigned long long V = grid;
-    const unsigned long long dep = V / (unsigned long long)a.tiles_per_plane;
-    a.dk = (int)(V % (unsigned long long)a.tiles_per_plane);
-    a.dpl = (int)(dep % (unsigned long long)g.planes);
-    a.dev = (int)(dep / (unsigned long long)g.planes);
-    if (pl.mode == 0) {     // the prologue synchronises the grid: co-residency guaranteed by a cooperative launch
+    // the kernel advances the tile counter by exactly n_tiles (n_tiles - grid tiles fetched + one failing fetch per CTA),
+    // and, in mode 1, the barrier counter by grid
+    a.tile_counter = ctx->d_counters + 4;
+    a.tile_base = ctx->tile_epoch;
+    a.dynamic_tiles = env_int("HT_FILL_DYNAMIC", 0) ? 1 : 0;     // measured equal on config 2 (53.2 vs 53.3 us); static keeps the launch deterministic
+    a.bar_count = ctx->d_counters + 5;
+    a.bar_target = ctx->bar_epoch + (pl.mode == 1 ? (uint32_t)grid : 0u);
+    {   // both prologues synchronise the grid: co-residency is guaranteed by a cooperative launch
         void *params[] = {&a};
         const void *fn = peaks ? reinterpret_cast<const void *>(ht::fill_tiles_kernel<true>)
                                : reinterpret_cast<const void *>(ht::fill_tiles_kernel<false>);
         HT_CUDA(cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(ht::kFillThreads), params, pl.smem, st));
-    } else {
-        if (peaks) ht::fill_tiles_kernel<true><<<(unsigned)grid, ht::kFillThreads, pl.smem, st>>>(a);
-        else ht::fill_tiles_kernel<false><<<(unsigned)grid, ht::kFillThreads, pl.smem, st>>>(a);
-        HT_CUDA(cudaGetLastError());
     }
+    if (a.dynamic_tiles) ctx->tile_epoch += (uint32_t)n_tiles;
+    ctx->bar_epoch = a.bar_target;
     ++ctx->launches;
     ctx->info[0] = (int32_t)grid; ctx->info[1] = ht::kFillThreads; ctx->info[2] = (int32_t)pl.smem;
     ctx->info[3] = rows_store; ctx->info[7] = pl.mode;
