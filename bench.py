@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
 
-A STEP is one pass of the whole hot path (classify+bucket, slab fill, peak scan+compaction: SURVEY.md section 8(a)
+A STEP is one pass of the whole hot path (classify, slab fill, peak test+compaction: SURVEY.md section 8(a)
 a0-a5) over one event of the workload (default: config 2, the paper-shaped 5000-hit event, 4x16x1024x1024 bins).
 `value` = events/s with the hits already resident in HBM (CUDA events on the launch stream, max over ranks);
 `e2e`   = the same metric through ht_run_host with pinned HOST buffers (H2D of the hits and D2H of the peak list inside
@@ -208,7 +208,10 @@ def bench_ours(args):
         for k in range(max(args.warmup, 3)):
             step(k)
         found = n_found_now()
-        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(n_marks)] for _ in range(args.steps)]
+        # one kernel per step: the bracketing events alone give its average duration (launch gap included); events
+        # between the two kernels of the split path are recorded only there (each record costs ~2 us of stream time)
+        inner = n_marks > 2
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(n_marks)] if inner else None for _ in range(args.steps)]
         l0 = B.ht_kernel_launches(ctx)
         barrier()
         if sampler is not None:
@@ -227,7 +230,10 @@ def bench_ours(args):
             t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             total_ms = float(t.item())
-        spans = [[e[i].elapsed_time(e[i + 1]) for e in evs] for i in range(n_marks - 1)]
+        if inner:
+            spans = [[e[i].elapsed_time(e[i + 1]) for e in evs] for i in range(n_marks - 1)]
+        else:
+            spans = [[total_ms / args.steps] * args.steps]
         return total_ms / args.steps, spans, launches, found
 
     fused_ok = True
@@ -275,8 +281,8 @@ def bench_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
     e2e_value = world * n_ev * e2e_steps / e2e_s
-    h2d = 3 * 4 * n_hits + 4 * (n_ev + 1)
-    d2h = 16 + 12 * min(cap, 1024)
+    h2d = 3 * 4 * n_hits + 4 * (n_ev + 1)                 # one packed copy: offsets + x + y + z
+    d2h = 4 + 12 * min(n_e2e, cap)                        # count + peak records, written by the kernel into mapped pinned memory
 
     if rank == 0:
         peak_gbs, peak_src = measured_hbm_peak()
@@ -293,11 +299,11 @@ def bench_ours(args):
         kernels, kernel_ms = {}, {}
         if "fused" in res:
             f = res["fused"][1][0]
-            kernels["ht_fill_peaks"] = roof("classify_bucket_kernel + fill_tiles_kernel<true> (ht_fill_peaks: classify, vote, store, peak test, compaction)",
+            kernels["ht_fill_peaks"] = roof("fill_tiles_kernel<true> (ht_fill_peaks: classify, vote, store, peak test, compaction in one kernel)",
                                             m_bytes + hit_bytes + pk_bytes, mean(f))
             kernel_ms.update(fused_median=statistics.median(f), fused_mean=mean(f), fused_step_mean=res["fused"][0])
         sp_fill, sp_peaks = res["split"][1]
-        kernels["ht_fill"] = roof("classify_bucket_kernel + fill_tiles_kernel<false> (ht_fill: classify, vote, store)", m_bytes + hit_bytes, mean(sp_fill))
+        kernels["ht_fill"] = roof("fill_tiles_kernel<false> (ht_fill: classify, vote, store in one kernel)", m_bytes + hit_bytes, mean(sp_fill))
         kernels["ht_peaks"] = roof("peaks_kernel (ht_peaks: scan+compaction)", m_bytes + pk_bytes, mean(sp_peaks))
         kernel_ms.update(fill_median=statistics.median(sp_fill), fill_mean=mean(sp_fill),
                          peaks_median=statistics.median(sp_peaks), peaks_mean=mean(sp_peaks),
@@ -392,7 +398,7 @@ def main():
         args.warmup = 1 if args.warmup is None else args.warmup
         bench_reference(args)
     else:
-        args.steps = 300 if args.steps is None else args.steps
+        args.steps = 2000 if args.steps is None else args.steps
         args.warmup = 10 if args.warmup is None else args.warmup
         bench_ours(args)
 

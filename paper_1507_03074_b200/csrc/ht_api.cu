@@ -115,12 +115,11 @@ struct ht_ctx {
     // peak scan launch geometry
     int peaks_unroll = 4, peaks_grid_vec4 = 0, peaks_grid_vec1 = 0;
     // host path (ht_run_host)
-    float *d_hx = nullptr, *d_hy = nullptr, *d_hz = nullptr;
-    int32_t *d_hoff = nullptr;
+    unsigned char *d_in = nullptr;     // [offsets | x | y | z], packed per call (one H2D copy)
+    unsigned char *h_in = nullptr;     // pinned mirror of d_in
     uint32_t *d_hmh = nullptr;
-    unsigned char *d_hres = nullptr;   // [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
-    unsigned char *h_res = nullptr;    // pinned mirror of d_hres
-    int32_t *h_off = nullptr;          // pinned staging of the per-group offsets
+    unsigned char *h_res = nullptr;    // pinned + mapped: [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
+    unsigned char *d_res = nullptr;    // device alias of h_res: the kernels write the peak list straight to the host
     cudaStream_t host_stream = nullptr;
     int64_t launches = 0;
     int32_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -145,12 +144,12 @@ WorkspaceSizes workspace_sizes(const ht_config *c)
     w.bucket_start = align_up(sizeof(int32_t) * (size_t)c->max_events * (planes + 1), 256);
     w.counts = align_up(sizeof(uint32_t) * (size_t)c->max_events * planes, 256);
     if (c->host_slots > 0) {
-        w.host_hits = 3 * align_up(sizeof(float) * (size_t)c->max_hits, 256);
-        w.host_off = align_up(sizeof(int32_t) * ((size_t)c->max_events + 1), 256);
+        w.host_hits = 3 * align_up(sizeof(float) * (size_t)c->max_hits, 16);
+        w.host_off = align_up(sizeof(int32_t) * ((size_t)c->max_events + 1), 16);
         w.host_mh = align_up(cells * sizeof(uint32_t) * (size_t)c->host_slots, 256);
         w.host_res = align_up(kResHeader + sizeof(ht_peak) * (size_t)c->host_peak_capacity, 256);
     }
-    w.total = w.tables + w.counters + w.buckets + w.bucket_start + w.counts + w.host_hits + w.host_off + w.host_mh + w.host_res;
+    w.total = w.tables + w.counters + w.buckets + w.bucket_start + w.counts + w.host_hits + w.host_off + w.host_mh;
     return w;
 }
 
@@ -267,17 +266,14 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
         return fail(cuda_fail(e, "table upload"));
 
     if (cfg->host_slots > 0) {
-        const size_t hb = align_up(sizeof(float) * (size_t)cfg->max_hits, 256);
-        if (!dmalloc((void **)&ctx->d_hx, w.host_hits, "cudaMalloc(host hits)")) return fail(rc);
-        ctx->d_hy = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ctx->d_hx) + hb);
-        ctx->d_hz = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ctx->d_hx) + 2 * hb);
-        if (!dmalloc((void **)&ctx->d_hoff, w.host_off, "cudaMalloc(host offsets)")) return fail(rc);
+        if (!dmalloc((void **)&ctx->d_in, w.host_off + w.host_hits, "cudaMalloc(host input)")) return fail(rc);
         if (!dmalloc((void **)&ctx->d_hmh, w.host_mh, "cudaMalloc(host matrices)")) return fail(rc);
-        if (!dmalloc((void **)&ctx->d_hres, w.host_res, "cudaMalloc(host result)")) return fail(rc);
-        if ((e = cudaMallocHost((void **)&ctx->h_res, w.host_res)) != cudaSuccess)
-            return fail(cuda_fail(e, "cudaMallocHost(result)"));
-        if ((e = cudaMallocHost((void **)&ctx->h_off, w.host_off)) != cudaSuccess)
-            return fail(cuda_fail(e, "cudaMallocHost(offsets)"));
+        if ((e = cudaMallocHost((void **)&ctx->h_in, w.host_off + w.host_hits)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaMallocHost(input)"));
+        if ((e = cudaHostAlloc((void **)&ctx->h_res, w.host_res, cudaHostAllocMapped)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaHostAlloc(result)"));
+        if ((e = cudaHostGetDevicePointer((void **)&ctx->d_res, ctx->h_res, 0)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaHostGetDevicePointer(result)"));
         if ((e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaStreamCreate"));
     }
@@ -548,50 +544,51 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
 
     cudaStream_t st = ctx->host_stream;
     const size_t cells = (size_t)ctx->geom.cells;
+    // input block [offsets | x | y | z], 16-byte aligned parts, packed in pinned memory: ONE host-to-device copy
+    const size_t o_x = align_up(sizeof(int32_t) * ((size_t)ctx->cfg.max_events + 1), 16);
+    const size_t part = align_up(sizeof(float) * (size_t)n_hits_total, 16);
+    const size_t o_y = o_x + part, o_z = o_y + part, in_bytes = o_z + part;
+    const float *d_x = reinterpret_cast<const float *>(ctx->d_in + o_x);
+    const float *d_y = reinterpret_cast<const float *>(ctx->d_in + o_y);
+    const float *d_z = reinterpret_cast<const float *>(ctx->d_in + o_z);
+    const int32_t *d_off = reinterpret_cast<const int32_t *>(ctx->d_in);
     if (n_hits_total > 0) {
         const size_t nb = sizeof(float) * (size_t)n_hits_total;
-        HT_CUDA(cudaMemcpyAsync(ctx->d_hx, h_x, nb, cudaMemcpyHostToDevice, st));
-        HT_CUDA(cudaMemcpyAsync(ctx->d_hy, h_y, nb, cudaMemcpyHostToDevice, st));
-        HT_CUDA(cudaMemcpyAsync(ctx->d_hz, h_z, nb, cudaMemcpyHostToDevice, st));
+        std::memcpy(ctx->h_in + o_x, h_x, nb);
+        std::memcpy(ctx->h_in + o_y, h_y, nb);
+        std::memcpy(ctx->h_in + o_z, h_z, nb);
     }
-    uint32_t *d_count = reinterpret_cast<uint32_t *>(ctx->d_hres);
-    ht_peak *d_list = reinterpret_cast<ht_peak *>(ctx->d_hres + kResHeader);
+    // the kernels write the count and the list straight into mapped pinned memory: no device-to-host copy
+    uint32_t *d_count = reinterpret_cast<uint32_t *>(ctx->d_res);
+    ht_peak *d_list = reinterpret_cast<ht_peak *>(ctx->d_res + kResHeader);
     uint32_t found_total = 0u, written = 0u;
     const int slots = ctx->cfg.host_slots;
-    int32_t *off_local = ctx->h_off;      // pinned; reused by the next group only after this group's synchronisation
+    int32_t *off_local = reinterpret_cast<int32_t *>(ctx->h_in);   // reused by the next group only after this group's synchronisation
     for (int e0 = 0; e0 < n_events; e0 += slots) {
         const int ne = (n_events - e0 < slots) ? n_events - e0 : slots;
         const int32_t hb = h_event_offsets[e0];
         for (int k = 0; k <= ne; ++k) off_local[k] = h_event_offsets[e0 + k] - hb;
         const int32_t nh = off_local[ne];
-        HT_CUDA(cudaMemcpyAsync(ctx->d_hoff, off_local, sizeof(int32_t) * (size_t)(ne + 1), cudaMemcpyHostToDevice, st));
+        if (e0 == 0)
+            HT_CUDA(cudaMemcpyAsync(ctx->d_in, ctx->h_in, in_bytes, cudaMemcpyHostToDevice, st));
+        else
+            HT_CUDA(cudaMemcpyAsync(ctx->d_in, ctx->h_in, sizeof(int32_t) * (size_t)(ne + 1), cudaMemcpyHostToDevice, st));
         const uint32_t room = capacity - written;
         // the fused kernel (matrix materialised AND peaks found in one pass); shapes it refuses take the two-call path
-        int rc = ht_fill_peaks(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, threshold,
-                               d_list, room, d_count, st);
+        int rc = ht_fill_peaks(ctx, d_x + hb, d_y + hb, d_z + hb, d_off, ne, nh, ctx->d_hmh, threshold, d_list, room, d_count, st);
         if (rc == HT_ERR_UNSUPPORTED) {
-            rc = ht_fill(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, st);
-            if (rc == HT_ERR_UNSUPPORTED)
-                rc = ht_fill_naive(ctx, ctx->d_hx + hb, ctx->d_hy + hb, ctx->d_hz + hb, ctx->d_hoff, ne, nh, ctx->d_hmh, st);
+            rc = ht_fill(ctx, d_x + hb, d_y + hb, d_z + hb, d_off, ne, nh, ctx->d_hmh, st);
+            if (rc == HT_ERR_UNSUPPORTED) rc = ht_fill_naive(ctx, d_x + hb, d_y + hb, d_z + hb, d_off, ne, nh, ctx->d_hmh, st);
             if (rc != HT_OK) return rc;
             rc = ht_peaks(ctx, ctx->d_hmh, ne, threshold, d_list, room, d_count, st);
         }
         if (rc != HT_OK) return rc;
-        // one D2H for count + a first slice of the list; a second one only if the list is longer than the slice
-        const uint32_t slice = room < 1024u ? room : 1024u;
-        HT_CUDA(cudaMemcpyAsync(ctx->h_res, ctx->d_hres, kResHeader + sizeof(ht_peak) * (size_t)slice, cudaMemcpyDeviceToHost, st));
         if (h_mh_or_null)
             HT_CUDA(cudaMemcpyAsync(h_mh_or_null + (size_t)e0 * cells, ctx->d_hmh, sizeof(uint32_t) * cells * (size_t)ne,
                                     cudaMemcpyDeviceToHost, st));
         HT_CUDA(cudaStreamSynchronize(st));
-        const uint32_t found = *reinterpret_cast<const uint32_t *>(ctx->h_res);
+        const uint32_t found = *reinterpret_cast<const volatile uint32_t *>(ctx->h_res);
         const uint32_t got = found < room ? found : room;
-        if (got > slice) {
-            HT_CUDA(cudaMemcpyAsync(ctx->h_res + kResHeader + sizeof(ht_peak) * (size_t)slice,
-                                    ctx->d_hres + kResHeader + sizeof(ht_peak) * (size_t)slice,
-                                    sizeof(ht_peak) * (size_t)(got - slice), cudaMemcpyDeviceToHost, st));
-            HT_CUDA(cudaStreamSynchronize(st));
-        }
         const ht_peak *src = reinterpret_cast<const ht_peak *>(ctx->h_res + kResHeader);
         for (uint32_t k = 0; k < got; ++k) {
             ht_peak p = src[k];
@@ -624,12 +621,10 @@ void ht_destroy(ht_ctx *ctx)
     cudaFree(ctx->d_bx);
     cudaFree(ctx->d_bucket_start);
     cudaFree(ctx->d_counts);
-    cudaFree(ctx->d_hx);
-    cudaFree(ctx->d_hoff);
+    cudaFree(ctx->d_in);
     cudaFree(ctx->d_hmh);
-    cudaFree(ctx->d_hres);
     if (ctx->h_res) cudaFreeHost(ctx->h_res);
-    if (ctx->h_off) cudaFreeHost(ctx->h_off);
+    if (ctx->h_in) cudaFreeHost(ctx->h_in);
     delete ctx;
 }
 
