@@ -165,7 +165,7 @@ struct FillPlan {
 size_t fill_smem_bytes(const ht_config &c, long long rows, int mode, long long n_hits)
 {
     const size_t slab = align_up((size_t)rows * (size_t)c.n_b * 4u, 16);
-    size_t b = 2u * slab + 4u * 4u * (size_t)(rows + 4);     // two slabs, two_a[4 ring entries][rows + 4]
+    size_t b = 2u * slab + 8u * 4u * (size_t)(rows + 4);     // two slabs, two_a[8 ring entries][rows + 4]
     b += align_up(4u * ((size_t)c.n_theta * (size_t)c.n_phi + 1u), 16);      // plane offsets, padded: the staged hits are float4
     if (mode == 1) b += 2u * (size_t)n_hits;
     return align_up(b, 16);
@@ -341,7 +341,15 @@ FillPlan plan_fill(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool pea
     // without the fused peak search the kernel is purely store-bound and measured fastest with slabs of <= 96 KB
     // (config 2, B200: 51.5 us at 96 KB, 53.4 at 100 KB, 59.4 at 104 KB); with it, the largest slab wins (fewer halo rows)
     const int slab_kb = env_int("HT_FILL_SLAB_KB", peaks ? 0 : 96);
+    // shared memory set aside for the hits the planner stages per tile (two buffers of 16 bytes per hit): room for twice
+    // the average number of hits per (event, plane), at most 512 hits; whatever else is left over is added below
+    long long want_cap = 2ll * (long long)n_hits / ((long long)(n_events > 0 ? n_events : 1) * planes);
+    want_cap = (want_cap + 31) / 32 * 32;
+    if (want_cap > 512) want_cap = 512;
+    if (want_cap < 32) want_cap = 32;
+    const size_t budget_all = budget;
     auto rows_for = [&](int md) -> long long {
+        const size_t budget = budget_all > (size_t)want_cap * 32u ? budget_all - (size_t)want_cap * 32u : 0;
         long long rows = c.n_a;
         if (slab_kb > 0 && rows > (long long)((size_t)slab_kb * 1024u / row_bytes)) rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
         if (rows < 1) rows = 1;
