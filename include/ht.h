@@ -14,8 +14,9 @@
  *
  * Conventions
  *   - Pointers named d_* are DEVICE pointers (on cfg.device), h_* are HOST pointers.  The caller owns every
- *     buffer it passes; the library owns only the ht_ctx (host struct + small device workspace: the angle tables
- *     and two counters; and, if cfg.host_slots > 0, staging buffers and host_slots vote matrices for ht_run_host).
+ *     buffer it passes; the library owns only the ht_ctx (host struct + small device workspace: the angle tables,
+ *     a few counters, per-hit scratch of the classification (20 bytes per hit of cfg.max_hits, 8 bytes per
+ *     (event, plane)); and, if cfg.host_slots > 0, staging buffers and host_slots vote matrices for ht_run_host).
  *   - Layout of a vote matrix (R15): uint32 M[event][itheta][iphi][ia][ib], ib fastest;
  *     cell = ((itheta*Nphi + iphi)*NA + ia)*NB + ib  (< 2^32 required).  d_mh must be 16-byte aligned.
  *   - ht_fill / ht_fill_peaks / ht_fill_naive / ht_peaks only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
@@ -93,10 +94,11 @@ HT_API int ht_create(const ht_config *cfg, ht_ctx **out);
  *   d_mh              device, n_events * cells uint32, FULLY OVERWRITTEN: every cell is stored exactly once
  *                     (zero or its count); it need not be cleared beforehand.  4-byte aligned; 16-byte alignment
  *                     (and n_b % 4 == 0) lets the rows leave as bulk (TMA) stores, otherwise plain stores are used.
- * One persistent kernel: each CTA owns a contiguous run of A rows of the batch, selects the hits of the current
- * (event, theta, phi) plane itself, builds tiles of rows as private shared-memory histograms and stores each tile
- * once: no global atomics, no memset pass, no workspace.
- * HT_ERR_UNSUPPORTED if one A row (n_b*4 bytes) does not fit the shared-memory tile (n_b > ~12000): ht_fill_naive.
+ * One persistent kernel (cooperative launch, one CTA per SM): the grid classifies every hit once into its
+ * (event, theta, phi) plane, then builds tiles of A rows as private shared-memory histograms (a warp owns a row) and
+ * stores each tile once with a bulk (TMA) copy: no global atomics on the matrix, no memset pass.
+ * HT_ERR_UNSUPPORTED if one A row (n_b*4 bytes) does not fit a shared-memory slab (two slabs share ~220 KB:
+ * n_b > ~27000), if the device cannot launch cooperatively, or if a batch has 2^31 tiles or more: ht_fill_naive.
  */
 HT_API int ht_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z,
                    const int32_t *d_event_offsets, int32_t n_events, int32_t n_hits_total, uint32_t *d_mh,
@@ -109,7 +111,8 @@ HT_API int ht_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float 
  * method; results are identical to ht_fill followed by ht_peaks.
  *   d_mh_or_null      as d_mh of ht_fill, or NULL: the matrices are not materialised at all (peaks only)
  *   threshold, d_out, capacity, d_n_found   as for ht_peaks
- * HT_ERR_UNSUPPORTED where ht_fill is, and if fewer than 2 A rows fit a tile (n_b > ~6000): use ht_fill + ht_peaks.
+ * HT_ERR_UNSUPPORTED where ht_fill is, and if fewer than 3 A rows fit a slab (one stored row plus the two
+ * neighbouring rows; n_b > ~9000): use ht_fill + ht_peaks.
  */
 HT_API int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z,
                          const int32_t *d_event_offsets, int32_t n_events, int32_t n_hits_total,
@@ -135,9 +138,11 @@ HT_API int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_
                     uint32_t capacity, uint32_t *d_n_found, void *cuda_stream);
 
 /*
- * End-to-end call with HOST buffers (needs cfg.host_slots >= 1): copies the hits to the device, runs ht_fill_peaks
- * (or ht_fill + ht_peaks where that is unsupported) on the context's own matrices (events in groups of host_slots),
- * copies the peak list and count back and synchronises.  h_out receives min(*h_n_found, capacity) records; capacity <= cfg.host_peak_capacity.
+ * End-to-end call with HOST buffers (needs cfg.host_slots >= 1): packs offsets and hits into one pinned block and
+ * copies it to the device (one transfer), runs ht_fill_peaks (or ht_fill + ht_peaks where that is unsupported) on the
+ * context's own matrices (events in groups of host_slots) with the peak list and count written by the kernel straight
+ * into mapped pinned memory, and synchronises.  h_out receives min(*h_n_found, capacity) records;
+ * capacity <= cfg.host_peak_capacity.
  * h_mh_or_null: if not NULL, n_events * cells uint32 that also receive the matrices (testing; slow).
  * Host buffers may be pageable or pinned (pinned makes the copies asynchronous DMA).
  */
@@ -149,7 +154,8 @@ HT_API int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const fl
 HT_API int64_t ht_kernel_launches(const ht_ctx *ctx);
 
 /* Launch geometry of the last ht_fill / ht_peaks (for DESIGN.md / bench reporting): out[0]=fill grid, out[1]=fill block,
- * out[2]=fill dynamic smem bytes, out[3]=rows per tile, out[4]=peaks grid, out[5]=peaks block, out[6]=SM count, out[7]=0. */
+ * out[2]=fill dynamic smem bytes, out[3]=rows stored per tile, out[4]=peaks grid, out[5]=peaks block, out[6]=SM count,
+ * out[7]=classification mode of the last fill (1: one event, hit index in shared memory; 0: batch, buckets in global memory). */
 HT_API int ht_launch_info(const ht_ctx *ctx, int32_t out[8]);
 
 /* Free everything the context owns.  NULL is allowed. */
