@@ -303,8 +303,8 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     }
     // peak scan: a persistent grid of exactly the CTAs that are resident at once (a grid-stride loop over more CTAs
     // than fit would run the excess as a second, partly empty wave)
-    int unroll = env_int("HT_PEAKS_UNROLL", 4);
-    if (unroll != 2 && unroll != 4 && unroll != 8) unroll = 4;
+    int unroll = env_int("HT_PEAKS_UNROLL", 2);      // config 2, B200, back-to-back launches: 45.2 us (U=2, 6 CTAs/SM), 46.4 (U=4), 49.4 (U=8)
+    if (unroll != 2 && unroll != 4 && unroll != 8) unroll = 2;
     ctx->peaks_unroll = unroll;
     int occ4 = 0, occ1 = 0;
     if (unroll == 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ4, ht::peaks_kernel<4, 2>, ht::kPeaksThreads, 0);

@@ -314,3 +314,33 @@ def test_error_codes_on_device_calls():
     cfg = B.ht_config.from_binning(bn, max_events=1, max_hits=1, device=99)
     with pytest.raises(B.HtError):
         B.ht_create(cfg)
+
+
+# ------------------------------------------------------------------ every code path of the fill kernel
+@pytest.mark.parametrize("env", [{"HT_FILL_MODE": "0"},            # batch classification (global buckets) on single events too
+                                 {"HT_FILL_DYNAMIC": "1"},          # tiles handed out through the global counter
+                                 {"HT_FILL_HIT_CAP": "32"},         # most hits bypass the shared-memory staging
+                                 {"HT_FILL_SLAB_KB": "8"},          # many small tiles, rows shared by few warps
+                                 {"HT_FILL_NO_BULK": "1"},          # plain stores instead of the TMA
+                                 {"HT_FILL_MODE": "0", "HT_FILL_DYNAMIC": "1", "HT_FILL_HIT_CAP": "0"}])
+def test_fill_kernel_variants_are_bit_exact(env, monkeypatch):
+    """The launch-time switches of the fill kernel (read from the environment at every call) change how the work is
+    organised, never the result."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    wl = WORKLOADS[2]
+    bn = Binning(4, 16, 256, 512)                                   # 33.5 M cells: the oracle takes a fraction of a second
+    one = generate_batch(wl, n_events=1)
+    assert _check_batch(bn, one, wl.threshold) > 0
+    three = generate_batch(WORKLOADS[3], n_events=3)
+    assert _check_batch(bn, three, wl.threshold) > 0
+
+
+def test_dense_tiles_with_many_peak_candidates():
+    """More candidates per tile than the store warp takes (32) and than a candidate list holds (128): the voters test
+    them, or scan the tile."""
+    wl = WORKLOADS[4]
+    bn = Binning(2, 2, 192, 256)                                    # 20000 hits in 4 planes: every tile is dense
+    batch = generate_batch(wl, n_events=1)
+    assert _check_batch(bn, batch, 3) > 1000
+    assert _check_batch(bn, generate_batch(wl, n_events=2), 40) > 0
