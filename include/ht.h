@@ -158,6 +158,12 @@ HT_API int64_t ht_kernel_launches(const ht_ctx *ctx);
  * out[7]=classification mode of the last fill (1: one event, hit index in shared memory; 0: batch, buckets in global memory). */
 HT_API int ht_launch_info(const ht_ctx *ctx, int32_t out[8]);
 
+/* Self-test of the arithmetic shortcut of the vote loop ("Exact division"): evaluates n_pairs
+ * pseudo-random quotients a/b (all significand patterns, exponents across and just outside the range the shortcut is
+ * used on) both ways on `device` and returns in *h_mismatches how many differ in any bit from __fdiv_rn (must be 0).
+ * Synchronous; allocates and frees 8 bytes of device memory. */
+HT_API int ht_selftest_division(int32_t device, uint64_t n_pairs, uint64_t seed, uint64_t *h_mismatches);
+
 /* Free everything the context owns.  NULL is allowed. */
 HT_API void ht_destroy(ht_ctx *ctx);
 

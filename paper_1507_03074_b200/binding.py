@@ -19,7 +19,7 @@ HT_OK, HT_ERR_INVALID_ARG, HT_ERR_UNSUPPORTED, HT_ERR_CUDA, HT_ERR_NOMEM = 0, -1
 PEAK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32)])   # == struct ht_peak
 
 EXPORTS = ("ht_query_sizes", "ht_tables_host", "ht_create", "ht_fill", "ht_fill_peaks", "ht_fill_naive", "ht_peaks", "ht_run_host",
-           "ht_kernel_launches", "ht_launch_info", "ht_destroy", "ht_strerror")
+           "ht_selftest_division", "ht_kernel_launches", "ht_launch_info", "ht_destroy", "ht_strerror")
 
 
 class ht_config(C.Structure):
@@ -76,6 +76,8 @@ def load() -> C.CDLL:
     lib.ht_peaks.argtypes = [vp, vp, i32, u32, vp, u32, vp, vp]
     lib.ht_run_host.restype = C.c_int
     lib.ht_run_host.argtypes = [vp, vp, vp, vp, vp, i32, i32, u32, vp, u32, vp, vp]
+    lib.ht_selftest_division.restype = C.c_int
+    lib.ht_selftest_division.argtypes = [i32, C.c_uint64, C.c_uint64, C.POINTER(C.c_uint64)]
     lib.ht_kernel_launches.restype = C.c_int64
     lib.ht_kernel_launches.argtypes = [vp]
     lib.ht_launch_info.restype = C.c_int
@@ -170,6 +172,13 @@ def ht_run_host(ctx, h_x, h_y, h_z, h_event_offsets, n_events: int, n_hits_total
     n = C.c_uint32(0)
     _check(load().ht_run_host(ctx, _ptr(h_x), _ptr(h_y), _ptr(h_z), _ptr(h_event_offsets), n_events, n_hits_total,
                               threshold, _ptr(h_out), capacity, C.addressof(n), _ptr(h_mh)), "ht_run_host")
+    return n.value
+
+
+def ht_selftest_division(device: int, n_pairs: int, seed: int) -> int:
+    """Number of quotients (out of n_pairs) for which the vote loop's division shortcut differs from __fdiv_rn."""
+    n = C.c_uint64(0)
+    _check(load().ht_selftest_division(device, n_pairs, seed, C.byref(n)), "ht_selftest_division")
     return n.value
 
 

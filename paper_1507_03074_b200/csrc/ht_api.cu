@@ -610,6 +610,25 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
     return HT_OK;
 }
 
+int ht_selftest_division(int32_t device, uint64_t n_pairs, uint64_t seed, uint64_t *h_mismatches)
+{
+    if (!h_mismatches) return HT_ERR_INVALID_ARG;
+    HT_CUDA(cudaSetDevice(device));
+    unsigned long long *d = nullptr;
+    HT_CUDA(cudaMalloc((void **)&d, sizeof(unsigned long long)));
+    cudaError_t e = cudaMemset(d, 0, sizeof(unsigned long long));
+    if (e == cudaSuccess) {
+        ht::selftest_division_kernel<<<148 * 8, 256>>>((unsigned long long)n_pairs, (unsigned long long)seed, d);
+        e = cudaGetLastError();
+    }
+    unsigned long long h = 0;
+    if (e == cudaSuccess) e = cudaMemcpy(&h, d, sizeof h, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(e, "ht_selftest_division");
+    *h_mismatches = (uint64_t)h;
+    return HT_OK;
+}
+
 int64_t ht_kernel_launches(const ht_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 int ht_launch_info(const ht_ctx *ctx, int32_t out[8])

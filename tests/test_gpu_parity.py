@@ -344,3 +344,10 @@ def test_dense_tiles_with_many_peak_candidates():
     batch = generate_batch(wl, n_events=1)
     assert _check_batch(bn, batch, 3) > 1000
     assert _check_batch(bn, generate_batch(wl, n_events=2), 40) > 0
+
+
+def test_division_shortcut_equals_fdiv_rn_on_four_billion_pairs():
+    """The vote loop divides with a hoisted reciprocal; on every pair it is used on it must give the
+    bits of the IEEE quotient.  4e9 pseudo-random pairs, exponents across and beyond the moderate range."""
+    assert B.ht_selftest_division(0, 4_000_000_000, 12345) == 0
+    assert B.ht_selftest_division(0, 100_000_000, 987654321) == 0
