@@ -371,7 +371,7 @@ def bench_ours(args):
                                        f"peaks {o_peaks * 1e3:.0f} ms), single thread, host of the GPU box",
                              "host_cpus": os.cpu_count()},
             "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "ht_run_host (pinned host buffers)"},
+                    "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "ht_run_host (host buffers -> pinned block; single event: the kernel reads the hits over PCIe (zero-copy), batches: one packed H2D copy; the peak list is written by the kernel into mapped pinned memory)"},
             "gpu_launches": int(launches),
             "clocks": sampler.summary(),
         }

@@ -138,8 +138,9 @@ HT_API int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_
                     uint32_t capacity, uint32_t *d_n_found, void *cuda_stream);
 
 /*
- * End-to-end call with HOST buffers (needs cfg.host_slots >= 1): packs offsets and hits into one pinned block and
- * copies it to the device (one transfer), runs ht_fill_peaks (or ht_fill + ht_peaks where that is unsupported) on the
+ * End-to-end call with HOST buffers (needs cfg.host_slots >= 1): packs offsets and hits into one pinned block, which
+ * the kernel reads directly (one event: every hit is read exactly once, zero-copy over PCIe) or which is copied to the
+ * device in one transfer (batches), runs ht_fill_peaks (or ht_fill + ht_peaks where that is unsupported) on the
  * context's own matrices (events in groups of host_slots) with the peak list and count written by the kernel straight
  * into mapped pinned memory, and synchronises.  h_out receives min(*h_n_found, capacity) records;
  * capacity <= cfg.host_peak_capacity.

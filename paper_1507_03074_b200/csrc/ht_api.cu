@@ -116,7 +116,8 @@ struct ht_ctx {
     int peaks_unroll = 4, peaks_grid_vec4 = 0, peaks_grid_vec1 = 0;
     // host path (ht_run_host)
     unsigned char *d_in = nullptr;     // [offsets | x | y | z], packed per call (one H2D copy)
-    unsigned char *h_in = nullptr;     // pinned mirror of d_in
+    unsigned char *h_in = nullptr;     // pinned + mapped mirror of d_in
+    unsigned char *d_in_mapped = nullptr;   // device alias of h_in (zero-copy input of single events)
     uint32_t *d_hmh = nullptr;
     unsigned char *h_res = nullptr;    // pinned + mapped: [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
     unsigned char *d_res = nullptr;    // device alias of h_res: the kernels write the peak list straight to the host
@@ -268,8 +269,10 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     if (cfg->host_slots > 0) {
         if (!dmalloc((void **)&ctx->d_in, w.host_off + w.host_hits, "cudaMalloc(host input)")) return fail(rc);
         if (!dmalloc((void **)&ctx->d_hmh, w.host_mh, "cudaMalloc(host matrices)")) return fail(rc);
-        if ((e = cudaMallocHost((void **)&ctx->h_in, w.host_off + w.host_hits)) != cudaSuccess)
-            return fail(cuda_fail(e, "cudaMallocHost(input)"));
+        if ((e = cudaHostAlloc((void **)&ctx->h_in, w.host_off + w.host_hits, cudaHostAllocMapped)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaHostAlloc(input)"));
+        if ((e = cudaHostGetDevicePointer((void **)&ctx->d_in_mapped, ctx->h_in, 0)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaHostGetDevicePointer(input)"));
         if ((e = cudaHostAlloc((void **)&ctx->h_res, w.host_res, cudaHostAllocMapped)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaHostAlloc(result)"));
         if ((e = cudaHostGetDevicePointer((void **)&ctx->d_res, ctx->h_res, 0)) != cudaSuccess)
@@ -556,10 +559,15 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
     const size_t o_x = align_up(sizeof(int32_t) * ((size_t)ctx->cfg.max_events + 1), 16);
     const size_t part = align_up(sizeof(float) * (size_t)n_hits_total, 16);
     const size_t o_y = o_x + part, o_z = o_y + part, in_bytes = o_z + part;
-    const float *d_x = reinterpret_cast<const float *>(ctx->d_in + o_x);
-    const float *d_y = reinterpret_cast<const float *>(ctx->d_in + o_y);
-    const float *d_z = reinterpret_cast<const float *>(ctx->d_in + o_z);
-    const int32_t *d_off = reinterpret_cast<const int32_t *>(ctx->d_in);
+    // One event whose hits the grid classifies in one pass (mode 1): the kernel reads every hit exactly once, so it reads
+    // them straight from the pinned block (zero-copy over PCIe) and no host-to-device copy is issued at all.
+    const bool zero_copy = n_events == 1 && env_int("HT_HOST_ZERO_COPY", 1) != 0 &&
+                           plan_fill(ctx, 1, n_hits_total, true).ok && plan_fill(ctx, 1, n_hits_total, true).mode == 1;
+    unsigned char *in_base = zero_copy ? ctx->d_in_mapped : ctx->d_in;
+    const float *d_x = reinterpret_cast<const float *>(in_base + o_x);
+    const float *d_y = reinterpret_cast<const float *>(in_base + o_y);
+    const float *d_z = reinterpret_cast<const float *>(in_base + o_z);
+    const int32_t *d_off = reinterpret_cast<const int32_t *>(in_base);
     if (n_hits_total > 0) {
         const size_t nb = sizeof(float) * (size_t)n_hits_total;
         std::memcpy(ctx->h_in + o_x, h_x, nb);
@@ -577,7 +585,9 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
         const int32_t hb = h_event_offsets[e0];
         for (int k = 0; k <= ne; ++k) off_local[k] = h_event_offsets[e0 + k] - hb;
         const int32_t nh = off_local[ne];
-        if (e0 == 0)
+        if (zero_copy)
+            ;
+        else if (e0 == 0)
             HT_CUDA(cudaMemcpyAsync(ctx->d_in, ctx->h_in, in_bytes, cudaMemcpyHostToDevice, st));
         else
             HT_CUDA(cudaMemcpyAsync(ctx->d_in, ctx->h_in, sizeof(int32_t) * (size_t)(ne + 1), cudaMemcpyHostToDevice, st));
