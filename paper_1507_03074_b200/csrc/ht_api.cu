@@ -141,7 +141,7 @@ WorkspaceSizes workspace_sizes(const ht_config *c)
     const size_t cells = planes * (size_t)c->n_a * (size_t)c->n_b;
     w.tables = align_up(sizeof(float) * (size_t)(c->n_theta + 1 + c->n_phi + 1), 256);
     w.counters = 256;
-    w.buckets = 5 * align_up(sizeof(float) * (size_t)c->max_hits, 256);      // bx, br2, bden, h_plane, h_rel
+    w.buckets = 6 * align_up(sizeof(float) * (size_t)c->max_hits, 256);      // hit records (4 words per hit), h_plane, h_rel
     w.bucket_start = align_up(sizeof(int32_t) * (size_t)c->max_events * (planes + 1), 256);
     w.counts = align_up(sizeof(uint32_t) * (size_t)c->max_events * planes, 256);
     if (c->host_slots > 0) {
@@ -252,11 +252,11 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     if (!dmalloc((void **)&ctx->d_bx, w.buckets, "cudaMalloc(hit buckets)")) return fail(rc);
     {
         unsigned char *b0 = reinterpret_cast<unsigned char *>(ctx->d_bx);
-        const size_t one = w.buckets / 5;
+        const size_t one = w.buckets / 6;
         ctx->d_br2 = reinterpret_cast<float *>(b0 + one);
         ctx->d_bden = reinterpret_cast<float *>(b0 + 2 * one);
-        ctx->d_hplane = reinterpret_cast<int32_t *>(b0 + 3 * one);
-        ctx->d_hrel = reinterpret_cast<int32_t *>(b0 + 4 * one);
+        ctx->d_hplane = reinterpret_cast<int32_t *>(b0 + 4 * one);
+        ctx->d_hrel = reinterpret_cast<int32_t *>(b0 + 5 * one);
     }
     if (!dmalloc((void **)&ctx->d_bucket_start, w.bucket_start, "cudaMalloc(bucket offsets)")) return fail(rc);
     if (!dmalloc((void **)&ctx->d_counts, w.counts, "cudaMalloc(bucket counts)")) return fail(rc);
