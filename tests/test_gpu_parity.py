@@ -351,3 +351,24 @@ def test_division_shortcut_equals_fdiv_rn_on_four_billion_pairs():
     bits of the IEEE quotient.  4e9 pseudo-random pairs, exponents across and beyond the moderate range."""
     assert B.ht_selftest_division(0, 4_000_000_000, 12345) == 0
     assert B.ht_selftest_division(0, 100_000_000, 987654321) == 0
+
+
+@pytest.mark.parametrize("zero_copy", ["1", "0"])
+def test_run_host_single_event_zero_copy_and_copy(zero_copy, monkeypatch):
+    """One event through ht_run_host: the kernel reads the hits straight from the pinned block (default) or the block is
+    copied to the device first; same matrix, same peaks, several calls in a row on one context."""
+    monkeypatch.setenv("HT_HOST_ZERO_COPY", zero_copy)
+    wl = WORKLOADS[2]
+    bn = Binning(4, 16, 256, 256)
+    with GpuHough(bn, 1, 6000, host_slots=1, host_peak_capacity=8192) as g:
+        for ev in range(3):
+            batch = generate_batch(wl, n_events=1, first_event=ev)
+            want_m = _oracle_batch(bn, batch)
+            want = oracle_peaks_batch(bn, want_m, wl.threshold)
+            out = np.zeros(8192, B.PEAK_DTYPE)
+            h_mh = np.full(bn.cells, 0xFFFFFFFF, np.uint32)
+            n = B.ht_run_host(g.ctx, batch.x, batch.y, batch.z, batch.event_offsets, 1, batch.n_hits, wl.threshold, out,
+                              8192, h_mh)
+            assert n == len(want) and n > 0
+            np.testing.assert_array_equal(sort_peaks(out[:n], bn.cells), want)
+            np.testing.assert_array_equal(h_mh.reshape(want_m[0].shape), want_m[0])
