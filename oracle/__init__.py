@@ -4,7 +4,7 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
 package.  It never imports the CUDA package, and the CUDA package never imports it.
 """
 from .ht_oracle import (OracleBinning, oracle_fill, oracle_fill_batch, oracle_peaks, oracle_peaks_batch,
-                        oracle_tables, oracle_votes, PEAK_DTYPE)
+                        oracle_tables, oracle_tracks, oracle_votes, PEAK_DTYPE)
 
 __all__ = ["OracleBinning", "oracle_fill", "oracle_fill_batch", "oracle_peaks", "oracle_peaks_batch",
-           "oracle_tables", "oracle_votes", "PEAK_DTYPE"]
+           "oracle_tables", "oracle_tracks", "oracle_votes", "PEAK_DTYPE"]

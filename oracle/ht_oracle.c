@@ -22,9 +22,10 @@
  * for every vote (P1), noiseless 12-layer track => one cell with 12 (P2), vote conservation (P3),
  * cell-centric brute force in double with atan2 binning on tiny binnings (P4), single-hit geometry (P5),
  * mirror symmetry (P6), permutation/batching invariance (P7), hand-built peak matrices (P8),
- * peak-set invariants (P9), table binning vs atan2 (P10), closed-form in-range fraction.
+ * peak-set invariants (P9), table binning vs atan2 (P10), closed-form in-range fraction; track read-out: the
+ * truth circle of a noiseless track (P11), polar identities and special cells (P12).
  * Parity unpinned by the paper (definitions fixed by SPEC.md only): R2/R4 angle definition and
- * ranges, R5 bin centre, R10 neighbourhood, R11 >= vs >, R12 tie rule.
+ * ranges, R5 bin centre, R10 neighbourhood, R11 >= vs >, R12 tie rule, R17 quadrant of phi.
  */
 #include <math.h>
 #include <stdint.h>
@@ -239,4 +240,33 @@ int64_t oracle_peaks(const oracle_binning *g, const uint32_t *M, uint32_t thresh
         }
     }
     return found;
+}
+
+/*
+ * Track read-out of a peak (SPEC.md section 4; "rho = sqrt(A^2 + B^2) and phi = tan^-1(B/A)"):
+ * (A, B) = centre of the peak's (A, B) cell = centre of the track's circle (the circle through the
+ * origin with centre (A, B) is x^2+y^2-2Ax-2By=0), so rho is the circle's radius and phi the azimuth of its
+ * centre.  Reading R17: tan^-1(B/A) is taken quadrant-aware (atan2), in (-pi, pi]; R18: (A, B) are the bin
+ * centres of R5, evaluated in binary32 exactly as the row values of the fill (they are inputs of the method,
+ * not results); rho and phi are then the PLAIN DEFINITION in double precision -- the CUDA path computes them
+ * in binary32 and is compared within a tolerance, no integer depends on them.
+ * Returns 0, or -1 on bad arguments.  Pins: P11 (truth circle of a noiseless track), P12 (identities).
+ */
+int oracle_tracks(const oracle_binning *g, const oracle_peak *peaks, int64_t n, double *rho, double *phi)
+{
+    if (!binning_ok(g) || n < 0 || (n > 0 && (!peaks || !rho || !phi))) return -1;
+    const float dA = (g->a_max - g->a_min) / (float)g->n_a;
+    const float dB = (g->b_max - g->b_min) / (float)g->n_b;
+    const uint64_t cells = (uint64_t)g->n_theta * g->n_phi * g->n_a * g->n_b;
+    for (int64_t k = 0; k < n; ++k) {
+        if (peaks[k].cell >= cells) return -1;
+        const uint32_t ib = peaks[k].cell % (uint32_t)g->n_b;
+        const uint32_t ia = (peaks[k].cell / (uint32_t)g->n_b) % (uint32_t)g->n_a;
+        const float fa = (float)ia + 0.5f, fb = (float)ib + 0.5f;
+        const float pa = fa * dA, pb = fb * dB;
+        const float A = g->a_min + pa, B = g->b_min + pb;          /* bin centres (R5, R18) */
+        rho[k] = sqrt((double)A * (double)A + (double)B * (double)B);
+        phi[k] = atan2((double)B, (double)A);
+    }
+    return 0;
 }

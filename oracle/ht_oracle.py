@@ -52,6 +52,9 @@ def _load():
         lib.oracle_peaks.restype = C.c_int64
         lib.oracle_peaks.argtypes = [C.POINTER(OracleBinning), C.POINTER(C.c_uint32), C.c_uint32, C.c_uint32,
                                      C.c_void_p, C.c_int64]
+        lib.oracle_tracks.restype = C.c_int
+        lib.oracle_tracks.argtypes = [C.POINTER(OracleBinning), C.c_void_p, C.c_int64, C.POINTER(C.c_double),
+                                      C.POINTER(C.c_double)]
         _lib = lib
     return _lib
 
@@ -141,3 +144,15 @@ def oracle_peaks_batch(binning, matrices, threshold: int) -> np.ndarray:
     """Concatenated peak list of a batch, sorted by (event, cell)."""
     parts = [oracle_peaks(binning, m, threshold, event=e) for e, m in enumerate(matrices)]
     return np.concatenate(parts) if parts else np.empty(0, PEAK_DTYPE)
+
+
+def oracle_tracks(binning, peaks: np.ndarray):
+    """(rho, phi) in float64 of every peak record (SPEC.md section 4)."""
+    g = OracleBinning.of(binning)
+    pk = np.ascontiguousarray(peaks, dtype=PEAK_DTYPE)
+    rho, phi = np.empty(len(pk), np.float64), np.empty(len(pk), np.float64)
+    dp = C.POINTER(C.c_double)
+    if _load().oracle_tracks(C.byref(g), pk.ctypes.data_as(C.c_void_p), len(pk), rho.ctypes.data_as(dp),
+                             phi.ctypes.data_as(dp)) != 0:
+        raise ValueError("oracle_tracks: invalid arguments (cell outside the matrix?)")
+    return rho, phi
