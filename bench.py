@@ -264,6 +264,20 @@ def bench_ours(args):
     ms_per_step, _, launches, _ = res[headline]
     value = world * n_ev * 1e3 / ms_per_step                          # events/s over all ranks
 
+    # ---- f3: track read-out (rho, phi) of the peak list, a separate small kernel (not part of the headline step)
+    d_tr = torch.empty(5 * cap, dtype=torch.int32, device=dev)
+    n_tr = min(n_found, cap)
+    for _ in range(5):
+        B.ht_tracks(ctx, d_out, n_tr, d_tr, stream)
+    stream.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(200):
+        B.ht_tracks(ctx, d_out, n_tr, d_tr, stream)
+    ev1.record(stream)
+    stream.synchronize()
+    tracks_ms = ev0.elapsed_time(ev1) / 200
+
     # ---- end to end through the host entry point: pinned host buffers, H2D + D2H inside the timed region
     hx, hy, hz = (torch.from_numpy(a.copy()).pin_memory() for a in (batch.x, batch.y, batch.z))
     hoff = torch.from_numpy(batch.event_offsets.copy()).pin_memory()
@@ -372,6 +386,7 @@ def bench_ours(args):
                              "host_cpus": os.cpu_count()},
             "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "ht_run_host (host buffers -> pinned block; single event: the kernel reads the hits over PCIe (zero-copy), batches: one packed H2D copy; the peak list is written by the kernel into mapped pinned memory)"},
+            "tracks": {"ms_per_call": tracks_ms, "n_peaks": n_tr, "what": "ht_tracks: rho, phi of every peak (f3), launch-bound"},
             "gpu_launches": int(launches),
             "clocks": sampler.summary(),
         }

@@ -137,6 +137,23 @@ HT_API int ht_fill_naive(ht_ctx *ctx, const float *d_x, const float *d_y, const 
 HT_API int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_t threshold, ht_peak *d_out,
                     uint32_t capacity, uint32_t *d_n_found, void *cuda_stream);
 
+/* A peak with the parameters of its track (f3). */
+typedef struct ht_track {
+    uint32_t event, cell, count; /* the peak record */
+    float rho;                   /* mm: radius of the track's circle = distance of the cell centre (A, B) from the origin */
+    float phi;                   /* rad, (-pi, pi]: azimuth of the circle's centre */
+} ht_track;
+
+/*
+ * Track read-out of a peak list ("rho = sqrt(A^2 + B^2) and phi = tan^-1(B/A)"; SPEC.md section 4):
+ * (A, B) = centre of the peak's cell = centre of the circle through the origin; phi is quadrant-aware (R17).
+ *   d_peaks   device, n_peaks records as written by ht_peaks / ht_fill_peaks (any order)
+ *   n_peaks   host value: min(count found, capacity of the list)
+ *   d_out     device, n_peaks ht_track records, same order as d_peaks
+ * Enqueues one small kernel on cuda_stream (binary32 arithmetic: rho within 2 ulp, phi within 4e-7 rad of the exact values).
+ */
+HT_API int ht_tracks(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, ht_track *d_out, void *cuda_stream);
+
 /*
  * End-to-end call with HOST buffers (needs cfg.host_slots >= 1): packs offsets and hits into one pinned block, which
  * the kernel reads directly (one event: every hit is read exactly once, zero-copy over PCIe) or which is copied to the

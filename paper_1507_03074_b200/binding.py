@@ -18,7 +18,10 @@ HT_OK, HT_ERR_INVALID_ARG, HT_ERR_UNSUPPORTED, HT_ERR_CUDA, HT_ERR_NOMEM = 0, -1
 
 PEAK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32)])   # == struct ht_peak
 
-EXPORTS = ("ht_query_sizes", "ht_tables_host", "ht_create", "ht_fill", "ht_fill_peaks", "ht_fill_naive", "ht_peaks", "ht_run_host",
+TRACK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32),
+                        ("rho", np.float32), ("phi", np.float32)])                                # == struct ht_track
+
+EXPORTS = ("ht_query_sizes", "ht_tables_host", "ht_create", "ht_fill", "ht_fill_peaks", "ht_fill_naive", "ht_peaks", "ht_tracks", "ht_run_host",
            "ht_selftest_division", "ht_kernel_launches", "ht_launch_info", "ht_destroy", "ht_strerror")
 
 
@@ -74,6 +77,8 @@ def load() -> C.CDLL:
     lib.ht_fill_peaks.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, u32, vp, u32, vp, vp]
     lib.ht_peaks.restype = C.c_int
     lib.ht_peaks.argtypes = [vp, vp, i32, u32, vp, u32, vp, vp]
+    lib.ht_tracks.restype = C.c_int
+    lib.ht_tracks.argtypes = [vp, vp, u32, vp, vp]
     lib.ht_run_host.restype = C.c_int
     lib.ht_run_host.argtypes = [vp, vp, vp, vp, vp, i32, i32, u32, vp, u32, vp, vp]
     lib.ht_selftest_division.restype = C.c_int
@@ -163,6 +168,11 @@ def ht_fill_naive(ctx, d_x, d_y, d_z, d_event_offsets, n_events: int, n_hits_tot
 def ht_peaks(ctx, d_mh, n_events: int, threshold: int, d_out, capacity: int, d_n_found, stream=None) -> None:
     _check(load().ht_peaks(ctx, _ptr(d_mh), n_events, threshold, _ptr(d_out), capacity, _ptr(d_n_found),
                            _stream(stream)), "ht_peaks")
+
+
+def ht_tracks(ctx, d_peaks, n_peaks: int, d_out, stream=None) -> None:
+    """(rho, phi) of n_peaks peak records: d_out receives n_peaks ht_track records (5 words each)."""
+    _check(load().ht_tracks(ctx, _ptr(d_peaks), n_peaks, _ptr(d_out), _stream(stream)), "ht_tracks")
 
 
 def ht_run_host(ctx, h_x, h_y, h_z, h_event_offsets, n_events: int, n_hits_total: int, threshold: int, h_out,

@@ -620,6 +620,20 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
     return HT_OK;
 }
 
+int ht_tracks(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, ht_track *d_out, void *cuda_stream)
+{
+    if (!ctx) return HT_ERR_INVALID_ARG;
+    if (n_peaks == 0u) return HT_OK;
+    if (!d_peaks || !d_out) return HT_ERR_INVALID_ARG;
+    static_assert(sizeof(ht::TrackOut) == sizeof(ht_track), "track record layout");
+    const unsigned threads = 128, blocks = (n_peaks + threads - 1u) / threads;
+    ht::tracks_kernel<<<blocks, threads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        reinterpret_cast<const ht::PeakOut *>(d_peaks), n_peaks, ctx->geom, reinterpret_cast<ht::TrackOut *>(d_out));
+    HT_CUDA(cudaGetLastError());
+    ++ctx->launches;
+    return HT_OK;
+}
+
 int ht_selftest_division(int32_t device, uint64_t n_pairs, uint64_t seed, uint64_t *h_mismatches)
 {
     if (!h_mismatches) return HT_ERR_INVALID_ARG;

@@ -372,3 +372,54 @@ def test_run_host_single_event_zero_copy_and_copy(zero_copy, monkeypatch):
             assert n == len(want) and n > 0
             np.testing.assert_array_equal(sort_peaks(out[:n], bn.cells), want)
             np.testing.assert_array_equal(h_mh.reshape(want_m[0].shape), want_m[0])
+
+
+# ------------------------------------------------------------------ f3: track read-out of the peaks
+def _tracks_gpu(g, pk):
+    dev = g.dev
+    rec = np.zeros((len(pk), 3), np.uint32)
+    rec[:, 0], rec[:, 1], rec[:, 2] = pk["event"], pk["cell"], pk["count"]
+    d_pk = torch.from_numpy(rec.view(np.int32)).to(dev)
+    d_out = torch.zeros(max(len(pk), 1) * 5, dtype=torch.int32, device=dev)
+    B.ht_tracks(g.ctx, d_pk, len(pk), d_out, None)
+    torch.cuda.synchronize()
+    return d_out[:5 * len(pk)].cpu().numpy().view(np.uint8).view(B.TRACK_DTYPE)
+
+
+def test_tracks_match_the_oracle_within_binary32_rounding():
+    """rho: products, sum and square root are each rounded once in binary32 (<= 2 ulp overall: rtol 2.4e-7); phi:
+    CUDA's atan2f is within 2 ulp, and |phi| < 4 has ulp 2.4e-7 (atol 6e-7).  DESIGN.md section 5.4."""
+    from oracle import oracle_tracks
+    wl = WORKLOADS[2]
+    bn = Binning(4, 16, 256, 512)
+    batch = generate_batch(wl, n_events=2)
+    want_m = _oracle_batch(bn, batch)
+    pk = oracle_peaks_batch(bn, want_m, wl.threshold)
+    assert len(pk) > 100
+    with GpuHough(bn, 2, batch.n_hits) as g:
+        # the peak list as the fused kernel writes it (its own order), read out on the device
+        _, n, got_pk = g.fill_peaks(batch, wl.threshold, store=False)
+        assert n == len(pk)
+        tr = _tracks_gpu(g, got_pk)
+        for f in ("event", "cell", "count"):
+            np.testing.assert_array_equal(tr[f], got_pk[f])
+        rho, phi = oracle_tracks(bn, got_pk)
+        np.testing.assert_allclose(tr["rho"].astype(np.float64), rho, rtol=2.4e-7, atol=0)
+        np.testing.assert_allclose(tr["phi"].astype(np.float64), phi, rtol=0, atol=6e-7)
+        assert len(_tracks_gpu(g, got_pk[:0])) == 0            # empty list: no launch, no error
+
+
+def test_tracks_every_cell_of_a_small_odd_binning():
+    """All cells, including the one at the origin (rho = 0, phi = 0), the axes and the four quadrants."""
+    from oracle import oracle_tracks
+    bn = Binning(2, 3, 9, 7, a_min=-9.0, a_max=9.0, b_min=-7.0, b_max=7.0)
+    pk = np.zeros(bn.cells, B.PEAK_DTYPE)
+    pk["cell"] = np.arange(bn.cells)
+    pk["count"] = 1
+    with GpuHough(bn, 1, 1) as g:
+        tr = _tracks_gpu(g, pk)
+    rho, phi = oracle_tracks(bn, pk)
+    np.testing.assert_allclose(tr["rho"].astype(np.float64), rho, rtol=2.4e-7, atol=0)
+    np.testing.assert_allclose(tr["phi"].astype(np.float64), phi, rtol=0, atol=6e-7)
+    origin = (4 * 7 + 3)
+    assert tr["rho"][origin] == 0.0 and tr["phi"][origin] == 0.0
