@@ -423,3 +423,33 @@ def test_tracks_every_cell_of_a_small_odd_binning():
     np.testing.assert_allclose(tr["phi"].astype(np.float64), phi, rtol=0, atol=6e-7)
     origin = (4 * 7 + 3)
     assert tr["rho"][origin] == 0.0 and tr["phi"][origin] == 0.0
+
+
+def test_seeded_random_shapes():
+    """40 seeded random binnings / batch shapes (ragged tiles, rows shared by several warps, NB % 4 != 0, empty events,
+    odd hit counts, partial angle ranges): matrix and peaks against the oracle, through all three call paths.
+    (Found: a misaligned table pointer for odd hit counts in the single-event classification.)"""
+    rng = np.random.default_rng(20241104)
+    for case in range(40):
+        n_theta, n_phi = int(rng.integers(1, 6)), int(rng.integers(1, 10))
+        n_a = int(rng.choice([1, 2, 3, 7, 31, 64, 100, 257]))
+        n_b = int(rng.choice([1, 4, 5, 12, 64, 250, 512, 700]))
+        kw = {}
+        if rng.random() < 0.3:
+            kw = dict(theta_min=0.3, theta_max=2.5, phi_min=0.5, phi_max=5.0)
+        if rng.random() < 0.3:
+            kw.update(a_min=-1500.0, a_max=2500.0, b_min=-3000.0, b_max=500.0)
+        bn = Binning(n_theta, n_phi, n_a, n_b, **kw)
+        n_events = int(rng.integers(1, 5))
+        events = []
+        for e in range(n_events):
+            n_hits = int(rng.choice([0, 1, 17, 300, 1500, int(rng.integers(1, 2500)), int(rng.integers(1, 2500))]))
+            xyz, _ = (np.zeros((0, 3), np.float32), None) if n_hits == 0 else \
+                __import__("paper_1507_03074_b200.events", fromlist=["generate_event"]).generate_event(
+                    int(rng.integers(1 << 30)), n_hits=n_hits, noise_frac=0.2)
+            events.append(xyz)
+        batch = batch_from_arrays(events)
+        if batch.n_hits == 0:
+            events[0] = np.array([[100.0, 50.0, 10.0]], np.float32)
+            batch = batch_from_arrays(events)
+        _check_batch(bn, batch, int(rng.integers(1, 7)))
