@@ -453,3 +453,20 @@ def test_seeded_random_shapes():
             events[0] = np.array([[100.0, 50.0, 10.0]], np.float32)
             batch = batch_from_arrays(events)
         _check_batch(bn, batch, int(rng.integers(1, 7)))
+
+
+@pytest.mark.parametrize("n_hits", [4999, 8193, 24577])
+def test_paper_binning_odd_and_boundary_hit_counts(n_hits):
+    """Full paper binning with odd hit counts and the counts at which the single-event classification changes its
+    register/scratch path (8192 hits) and gives way to the batch path (24576 hits)."""
+    from paper_1507_03074_b200.events import generate_event
+    bn = WORKLOADS[2].binning
+    xyz, _ = generate_event(777 + n_hits, n_hits=n_hits, noise_frac=0.1)
+    batch = batch_from_arrays([xyz])
+    want_m = _oracle_batch(bn, batch)
+    want_p = oracle_peaks_batch(bn, want_m, 9)
+    with GpuHough(bn, 1, batch.n_hits) as g:
+        mh, n, pk = g.fill_peaks(batch, 9)
+        assert n == len(want_p)
+        np.testing.assert_array_equal(sort_peaks(pk, bn.cells), want_p)
+        assert torch.equal(mh.cpu(), torch.from_numpy(want_m[0].reshape(-1).view(np.int32)))
