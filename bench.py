@@ -11,7 +11,8 @@ a0-a5) over one event of the workload (default: config 2, the paper-shaped 5000-
 `roofline` = achieved HBM GB/s of the dominant kernel call (algorithmic bytes / CUDA-event duration measured in the
           timed region) against MEASURED_PEAKS.json;
 `cpu_baseline` = the CPU oracle as it stands, one core, on the same event (also checks parity in the same run).
-N > 1 (torchrun): every rank processes its own seeded event, no data-path collective ("scaling": "weak").
+N > 1 (torchrun): every rank processes its own seeded event, no data-path collective ("scaling": "weak"); with
+`--split planes` all ranks take the same event and a range of (theta, phi) planes each ("strong").
 `--impl reference` times the CPU oracle itself (there is no reference implementation of the paper to install).
 """
 from __future__ import annotations
@@ -149,12 +150,19 @@ def bench_ours(args):
     bn = wl.binning
     n_ev = args.events if args.events else 1
     # every rank its own events (weak scaling: the path shards by event, no data-path collective)
-    batch = generate_batch(wl, n_events=n_ev, first_event=rank * n_ev)
+    # --split events (default): every rank its own events (weak scaling: the path shards by event, no data-path
+    # collective).  --split planes: all ranks take the SAME events and a contiguous range of the (theta, phi) planes each
+    # (strong scaling; the sector split of PAPER.md:77); again no collective in the timed region
+    by_planes = args.split == "planes"
+    batch = generate_batch(wl, n_events=n_ev, first_event=0 if by_planes else rank * n_ev)
     n_hits = batch.n_hits
-    cells = bn.cells
+    from paper_1507_03074_b200.sharding import plane_range
+    p0, pc = plane_range(bn.planes, rank, world) if by_planes else (0, bn.planes)
+    cells = pc * bn.n_a * bn.n_b                                     # cells of this rank's matrix per event
     cap = 1 << 16
     cfg = B.ht_config.from_binning(bn, max_events=n_ev, max_hits=n_hits, device=local_rank, host_slots=n_ev,
-                                   host_peak_capacity=cap)
+                                   host_peak_capacity=cap, plane_begin=p0 if by_planes else 0,
+                                   plane_count=pc if by_planes else 0)
     ctx = B.ht_create(cfg)
     stream = torch.cuda.Stream(device=dev)
 
@@ -262,7 +270,8 @@ def bench_ours(args):
     (step_fused if headline == "fused" else step_split)(last_k)
     n_found = n_found_now()
     ms_per_step, _, launches, _ = res[headline]
-    value = world * n_ev * 1e3 / ms_per_step                          # events/s over all ranks
+    jobs = 1 if by_planes else world                                  # --split planes: all ranks work on the same events
+    value = jobs * n_ev * 1e3 / ms_per_step                           # events/s over all ranks
 
     # ---- f3: track read-out (rho, phi) of the peak list, a separate small kernel (not part of the headline step)
     d_tr = torch.empty(5 * cap, dtype=torch.int32, device=dev)
@@ -294,7 +303,7 @@ def bench_ours(args):
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
-    e2e_value = world * n_ev * e2e_steps / e2e_s
+    e2e_value = jobs * n_ev * e2e_steps / e2e_s
     h2d = 3 * 4 * n_hits + 4 * (n_ev + 1)                 # one packed copy: offsets + x + y + z
     d2h = 4 + 12 * min(n_e2e, cap)                        # count + peak records, written by the kernel into mapped pinned memory
 
@@ -343,7 +352,8 @@ def bench_ours(args):
         k = min(n_found, cap)
         rec = d_out[:3 * k].cpu().numpy().view(np.uint32).reshape(k, 3)
         rec = rec[np.lexsort((rec[:, 1], rec[:, 0]))]
-        parity = bool(np.array_equal(got_all[0], m_ref.reshape(-1)))
+        lo_cell, hi_cell = p0 * bn.n_a * bn.n_b, (p0 + pc) * bn.n_a * bn.n_b     # this rank's part of the full matrix
+        parity = bool(np.array_equal(got_all[0], m_ref.reshape(-1)[lo_cell:hi_cell]))
         n_ref, votes_all = 0, 0
         for e in range(n_ev):
             if e == 0:
@@ -351,8 +361,9 @@ def bench_ours(args):
             else:
                 m_e, v_e = oracle_fill(bn, *batch.event(e))
                 pk_e = oracle_peaks(bn, m_e, T)
-                parity = parity and bool(np.array_equal(got_all[e], m_e.reshape(-1)))
+                parity = parity and bool(np.array_equal(got_all[e], m_e.reshape(-1)[lo_cell:hi_cell]))
             votes_all += v_e
+            pk_e = pk_e[(pk_e["cell"] >= lo_cell) & (pk_e["cell"] < hi_cell)]
             r_e = rec[rec[:, 0] == e]
             parity = parity and len(r_e) == len(pk_e) and bool(np.array_equal(r_e[:, 1], pk_e["cell"])
                                                                 and np.array_equal(r_e[:, 2], pk_e["count"]))
@@ -365,7 +376,8 @@ def bench_ours(args):
         info = B.ht_launch_info(ctx)
         line = {
             "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "strong" if by_planes else "weak",
             "vs_baseline": None, "dtype": "u32 counts / f32 bin decisions", "data": "synthetic",
             "config": {"workload": f"config{wl.config}:{wl.name}", "bins": [bn.n_theta, bn.n_phi, bn.n_a, bn.n_b],
                        "hits_per_step": n_hits, "threshold": T, "events_per_step": n_ev,
@@ -374,11 +386,11 @@ def bench_ours(args):
                        "l2": f"M_H per step ({m_bytes / 1e6:.0f} MB) is larger than the 126 MB L2; {n_rot} output matrices "
                              "rotated so no step inherits another step's lines",
                        "launch": info},
-            "votes_per_s": votes_all * world * 1e3 / ms_per_step, "votes_per_step": votes_all, "peaks_per_step": n_found,
-            "hit_a_evaluations_per_s": n_hits * bn.n_a * world * 1e3 / ms_per_step,
+            "votes_per_s": votes_all * jobs * 1e3 / ms_per_step, "votes_per_step": votes_all, "peaks_per_step": n_found,
+            "hit_a_evaluations_per_s": n_hits * bn.n_a * jobs * 1e3 / ms_per_step,
             "parity_vs_oracle": "bit-exact" if parity else "MISMATCH",
             "kernel_ms": kernel_ms,
-            "paths_events_per_s": {name: world * n_ev * 1e3 / r[0] for name, r in res.items()},
+            "paths_events_per_s": {name: jobs * n_ev * 1e3 / r[0] for name, r in res.items()},
             "roofline": dominant, "roofline_kernels": kernels,
             "cpu_baseline": {"value": 1.0 / (o_fill + o_peaks), "unit": "events/s", "cores": 1, "kind": "oracle",
                              "sample": f"median of {reps} runs of one full event of this workload (fill {o_fill * 1e3:.0f} ms + "
@@ -411,6 +423,8 @@ def main():
     ap.add_argument("--mode", choices=["fused", "split"], default="fused",
                     help="headline path: ht_fill_peaks (one kernel) or ht_fill + ht_peaks")
     ap.add_argument("--rotate", type=int, default=4, help="number of output matrices rotated between steps")
+    ap.add_argument("--split", choices=["events", "planes"], default="events",
+                    help="N > 1: every rank its own events (weak scaling, default) or the same events split by plane")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = 10 if args.steps is None else args.steps

@@ -19,6 +19,7 @@
  *     (event, plane)); and, if cfg.host_slots > 0, staging buffers and host_slots vote matrices for ht_run_host).
  *   - Layout of a vote matrix (R15): uint32 M[event][itheta][iphi][ia][ib], ib fastest;
  *     cell = ((itheta*Nphi + iphi)*NA + ia)*NB + ib  (< 2^32 required).  d_mh must be 16-byte aligned.
+ *     A context with a plane range (cfg.plane_count > 0) holds only its planes: M[event][plane - plane_begin][ia][ib].
  *   - ht_fill / ht_fill_peaks / ht_fill_naive / ht_peaks only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
  *     void*, e.g. torch.cuda.Stream().cuda_stream; NULL = the legacy default stream).  No host
  *     synchronisation, no allocation.  Results are valid once the caller has synchronised the stream.
@@ -67,6 +68,12 @@ typedef struct ht_config {
     int32_t device;                    /* CUDA ordinal */
     int32_t host_slots;                /* >= 0: vote matrices owned by the context for ht_run_host (0: that call is unavailable) */
     uint32_t host_peak_capacity;       /* peak-list capacity of the context's staging buffer for ht_run_host */
+    /* Plane range of this context (f2; the sector split of PAPER.md:77 "four M_H(A,B,theta), each matrix processing the
+     * data of a single phi sector"): the context fills and scans only the (theta,phi) planes
+     * [plane_begin, plane_begin + plane_count) of the n_theta * n_phi (plane = itheta * n_phi + iphi); hits of other
+     * planes are ignored; its matrices hold plane_count planes per event; peak records carry the cell index of the
+     * FULL matrix.  plane_count == 0: all planes. */
+    int32_t plane_begin, plane_count;
 } ht_config;
 
 typedef struct ht_peak {

@@ -30,17 +30,21 @@ class ht_config(C.Structure):
                 ("a_min", C.c_float), ("a_max", C.c_float), ("b_min", C.c_float), ("b_max", C.c_float),
                 ("theta_min", C.c_float), ("theta_max", C.c_float), ("phi_min", C.c_float), ("phi_max", C.c_float),
                 ("max_events", C.c_int32), ("max_hits", C.c_int32), ("device", C.c_int32),
-                ("host_slots", C.c_int32), ("host_peak_capacity", C.c_uint32)]
+                ("host_slots", C.c_int32), ("host_peak_capacity", C.c_uint32),
+                ("plane_begin", C.c_int32), ("plane_count", C.c_int32)]
 
     @classmethod
     def from_binning(cls, b, *, max_events: int, max_hits: int, device: int = 0, host_slots: int = 0,
-                     host_peak_capacity: int = 0) -> "ht_config":
+                     host_peak_capacity: int = 0, plane_begin: int = 0, plane_count: int = 0) -> "ht_config":
         return cls(b.n_theta, b.n_phi, b.n_a, b.n_b, b.a_min, b.a_max, b.b_min, b.b_max, b.theta_min, b.theta_max,
-                   b.phi_min, b.phi_max, max_events, max_hits, device, host_slots, host_peak_capacity)
+                   b.phi_min, b.phi_max, max_events, max_hits, device, host_slots, host_peak_capacity, plane_begin,
+                   plane_count)
 
     @property
     def cells(self) -> int:
-        return self.n_theta * self.n_phi * self.n_a * self.n_b
+        """Cells of one event's matrix IN THIS CONTEXT (its plane range only)."""
+        planes = self.plane_count if self.plane_count > 0 else self.n_theta * self.n_phi
+        return planes * self.n_a * self.n_b
 
 
 class HtError(RuntimeError):

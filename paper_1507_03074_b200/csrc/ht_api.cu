@@ -50,6 +50,9 @@ bool config_ok(const ht_config *c)
         (unsigned long long)c->n_theta * (unsigned long long)c->n_phi * (unsigned long long)c->n_a * (unsigned long long)c->n_b;
     if (cells >= (1ull << 32)) return false;          // ht_peak.cell is uint32
     if ((long long)c->n_theta * (long long)c->n_phi > (1ll << 30)) return false;
+    if (c->plane_begin < 0 || c->plane_count < 0) return false;
+    if (c->plane_count > 0 && (long long)c->plane_begin + c->plane_count > (long long)c->n_theta * c->n_phi) return false;
+    if (c->plane_count == 0 && c->plane_begin != 0) return false;
     return true;
 }
 
@@ -138,7 +141,7 @@ WorkspaceSizes workspace_sizes(const ht_config *c)
 {
     WorkspaceSizes w{};
     const size_t planes = (size_t)c->n_theta * (size_t)c->n_phi;
-    const size_t cells = planes * (size_t)c->n_a * (size_t)c->n_b;
+    const size_t cells = (c->plane_count > 0 ? (size_t)c->plane_count : planes) * (size_t)c->n_a * (size_t)c->n_b;
     w.tables = align_up(sizeof(float) * (size_t)(c->n_theta + 1 + c->n_phi + 1), 256);
     w.counters = 256;
     w.buckets = 6 * align_up(sizeof(float) * (size_t)c->max_hits, 256);      // hit records (4 words per hit), h_plane, h_rel
@@ -192,7 +195,8 @@ extern "C" {
 int ht_query_sizes(const ht_config *cfg, size_t *mh_bytes_per_event, size_t *ctx_device_bytes)
 {
     if (!config_ok(cfg) || cfg->max_events < 1 || cfg->max_hits < 1 || cfg->host_slots < 0) return HT_ERR_INVALID_ARG;
-    const size_t cells = (size_t)cfg->n_theta * (size_t)cfg->n_phi * (size_t)cfg->n_a * (size_t)cfg->n_b;
+    const size_t planes = cfg->plane_count > 0 ? (size_t)cfg->plane_count : (size_t)cfg->n_theta * (size_t)cfg->n_phi;
+    const size_t cells = planes * (size_t)cfg->n_a * (size_t)cfg->n_b;
     if (mh_bytes_per_event) *mh_bytes_per_event = cells * sizeof(uint32_t);
     if (ctx_device_bytes) *ctx_device_bytes = workspace_sizes(cfg).total;
     return HT_OK;
@@ -220,8 +224,10 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     ctx->cfg = *cfg;
     ht::Geom &g = ctx->geom;
     g.n_theta = cfg->n_theta; g.n_phi = cfg->n_phi; g.n_a = cfg->n_a; g.n_b = cfg->n_b;
-    g.planes = cfg->n_theta * cfg->n_phi;
+    g.planes = cfg->plane_count > 0 ? cfg->plane_count : cfg->n_theta * cfg->n_phi;
+    g.plane0 = cfg->plane_count > 0 ? cfg->plane_begin : 0;
     g.cells = (unsigned long long)g.planes * (unsigned long long)cfg->n_a * (unsigned long long)cfg->n_b;
+    g.cell_base = (uint32_t)((unsigned long long)g.plane0 * (unsigned long long)cfg->n_a * (unsigned long long)cfg->n_b);
     std::vector<float> tth((size_t)cfg->n_theta + 1), pph((size_t)cfg->n_phi + 1);
     float d_ab[2];
     build_tables(cfg, nullptr, tth.data(), pph.data(), d_ab);

@@ -79,3 +79,13 @@ def gather_peaks(local_peaks: np.ndarray, first_event: int, cells: int, group=No
         p["event"], p["cell"], p["count"] = a[:, 0], a[:, 1], a[:, 2]
         parts.append(p)
     return sort_peaks(np.concatenate(parts) if parts else np.empty(0, PEAK_DTYPE), cells)
+
+
+def plane_range(n_planes: int, rank: int, world: int) -> tuple[int, int]:
+    """(plane_begin, plane_count) of ``rank`` when ONE event is split over the ranks by (theta, phi) plane -- the sector
+    split of PAPER.md:77 ("four M_H(A,B,theta), each matrix processing the data of a single phi sector"), generalised to
+    any contiguous block of planes (plane = itheta * n_phi + iphi).  Planes never exchange votes or peaks (R10), so every
+    rank gets all the hits, fills and scans its planes (``ht_config.plane_begin / plane_count``), and the only
+    communication is ``gather_peaks`` (``first_event = 0``: the records already carry full-matrix cell indices)."""
+    first, last = event_range(n_planes, rank, world)
+    return first, last - first

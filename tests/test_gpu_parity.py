@@ -470,3 +470,51 @@ def test_paper_binning_odd_and_boundary_hit_counts(n_hits):
         assert n == len(want_p)
         np.testing.assert_array_equal(sort_peaks(pk, bn.cells), want_p)
         assert torch.equal(mh.cpu(), torch.from_numpy(want_m[0].reshape(-1).view(np.int32)))
+
+
+# ------------------------------------------------------------------ f2: one event split over contexts by (theta, phi) plane
+@pytest.mark.parametrize("world", [2, 3, 4])
+def test_plane_ranges_reassemble_the_full_result(world):
+    """one matrix per sector.  `world` contexts (one per would-be GPU, here one after the other on one
+    device) take contiguous plane ranges; their matrices are the plane slices of the oracle's matrix and their peak lists
+    -- full-matrix cell indices -- add up to the oracle's, through ht_fill + ht_peaks and through ht_fill_peaks."""
+    from paper_1507_03074_b200.sharding import plane_range
+    wl = WORKLOADS[2]
+    bn = Binning(3, 5, 200, 256)
+    batch = generate_batch(wl, n_events=2)
+    want_m = _oracle_batch(bn, batch)
+    want_p = oracle_peaks_batch(bn, want_m, wl.threshold)
+    dev = torch.device("cuda:0")
+    parts_split, parts_fused = [], []
+    for rank in range(world):
+        p0, pc = plane_range(bn.planes, rank, world)
+        cfg = B.ht_config.from_binning(bn, max_events=2, max_hits=batch.n_hits, device=0, plane_begin=p0, plane_count=pc)
+        assert B.ht_query_sizes(cfg)[0] == 4 * pc * bn.n_a * bn.n_b
+        ctx = B.ht_create(cfg)
+        try:
+            to = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dtype=dt)
+            dx, dy, dz, doff = (to(batch.x, torch.float32), to(batch.y, torch.float32), to(batch.z, torch.float32),
+                                to(batch.event_offsets, torch.int32))
+            cells = cfg.cells
+            out = torch.zeros(3 << 14, dtype=torch.int32, device=dev)
+            nf = torch.zeros(1, dtype=torch.int32, device=dev)
+            for fused in (False, True):
+                mh = torch.full((2 * cells,), -1, dtype=torch.int32, device=dev)
+                if fused:
+                    B.ht_fill_peaks(ctx, dx, dy, dz, doff, 2, batch.n_hits, mh, wl.threshold, out, 1 << 14, nf, None)
+                else:
+                    B.ht_fill(ctx, dx, dy, dz, doff, 2, batch.n_hits, mh, None)
+                    B.ht_peaks(ctx, mh, 2, wl.threshold, out, 1 << 14, nf, None)
+                torch.cuda.synchronize()
+                got = mh.cpu().numpy().view(np.uint32).reshape(2, pc, bn.n_a, bn.n_b)
+                for e in range(2):
+                    np.testing.assert_array_equal(got[e], want_m[e].reshape(bn.planes, bn.n_a, bn.n_b)[p0:p0 + pc])
+                n = int(nf.cpu().numpy().view(np.uint32)[0])
+                rec = out[:3 * n].cpu().numpy().view(np.uint32).reshape(n, 3)
+                pk = np.empty(n, B.PEAK_DTYPE)
+                pk["event"], pk["cell"], pk["count"] = rec[:, 0], rec[:, 1], rec[:, 2]
+                (parts_fused if fused else parts_split).append(pk)
+        finally:
+            B.ht_destroy(ctx)
+    for parts in (parts_split, parts_fused):
+        np.testing.assert_array_equal(sort_peaks(np.concatenate(parts), bn.cells), want_p)

@@ -17,7 +17,7 @@ import torch.multiprocessing as mp
 from oracle import oracle_fill, oracle_peaks, oracle_peaks_batch
 from paper_1507_03074_b200.binding import PEAK_DTYPE
 from paper_1507_03074_b200.events import Binning, Workload, generate_batch
-from paper_1507_03074_b200.sharding import event_range, gather_peaks, rebase_peaks, shard_batch, sort_peaks
+from paper_1507_03074_b200.sharding import event_range, gather_peaks, plane_range, rebase_peaks, shard_batch, sort_peaks
 
 BN = Binning(2, 4, 64, 64)
 WL = Workload(1, "tiny_sharded", BN, n_events=5, threshold=6, n_tracks=12)
@@ -97,3 +97,11 @@ def test_gather_without_a_process_group_is_the_identity():
     p["event"], p["cell"], p["count"] = [0, 0], [7, 3], [9, 9]
     q = gather_peaks(p, 4, cells=64)
     assert q["event"].tolist() == [4, 4] and q["cell"].tolist() == [3, 7]
+
+
+def test_plane_ranges_partition_the_planes():
+    for n_planes in (1, 4, 15, 64, 256):
+        for world in (1, 2, 3, 4, 8):
+            spans = [plane_range(n_planes, r, world) for r in range(world)]
+            assert spans[0][0] == 0 and sum(c for _, c in spans) == n_planes
+            assert all(spans[r][0] + spans[r][1] == spans[r + 1][0] for r in range(world - 1))
