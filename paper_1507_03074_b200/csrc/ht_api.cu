@@ -112,7 +112,7 @@ struct ht_ctx {
     uint32_t *d_counts = nullptr;          // [max_events * P], zero between calls
     // tile fill launch geometry: per-kernel dynamic shared memory budget ([0]: ht_fill, [1]: fused peaks), and whether
     // the device can run the kernel at all (one CTA of 1024 threads per SM, cooperative launch for mode 0)
-    uint32_t bar_epoch = 0, tile_epoch = 0;   // host mirrors of the two device counters that only grow (d_counters[4], [5])
+    uint32_t bar_epoch = 0;                   // host mirror of the barrier counter that only grows (d_counters[5])
     bool fill_ok = false;
     size_t fill_smem_max[2] = {0, 0};
     // peak scan launch geometry
@@ -440,21 +440,20 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     unsigned long long grid = (unsigned long long)ctx->sm_count;
     if (grid > n_tiles) grid = n_tiles;
     if (grid < 1) grid = 1;
-    // the kernel advances the tile counter by exactly n_tiles (n_tiles - grid tiles fetched + one failing fetch per CTA),
-    // and, in mode 1, the barrier counter by grid
-    a.tile_counter = ctx->d_counters + 4;
-    a.tile_base = ctx->tile_epoch;
-    a.dynamic_tiles = env_int("HT_FILL_DYNAMIC", 0) ? 1 : 0;     // measured equal on config 2 (53.2 vs 53.3 us); static keeps the launch deterministic
-    a.bar_count = ctx->d_counters + 5;
-    a.bar_target = ctx->bar_epoch + (pl.mode == 1 ? (uint32_t)grid : 0u);
+    // Mode 1's grid barrier: the fast one-shot form needs the host to know the counter's value, which a launch captured
+    // into a CUDA graph (replayed any number of times) cannot; captured launches use the self-resetting barrier.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    HT_CUDA(cudaStreamIsCapturing(st, &cap));
+    const bool one_shot = pl.mode == 1 && cap == cudaStreamCaptureStatusNone;
+    a.bar_count = one_shot ? ctx->d_counters + 5 : nullptr;
+    a.bar_target = ctx->bar_epoch + (uint32_t)grid;
     {   // both prologues synchronise the grid: co-residency is guaranteed by a cooperative launch
         void *params[] = {&a};
         const void *fn = peaks ? reinterpret_cast<const void *>(ht::fill_tiles_kernel<true>)
                                : reinterpret_cast<const void *>(ht::fill_tiles_kernel<false>);
         HT_CUDA(cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(ht::kFillThreads), params, pl.smem, st));
     }
-    if (a.dynamic_tiles) ctx->tile_epoch += (uint32_t)n_tiles;
-    ctx->bar_epoch = a.bar_target;
+    if (one_shot) ctx->bar_epoch = a.bar_target;
     ++ctx->launches;
     ctx->info[0] = (int32_t)grid; ctx->info[1] = ht::kFillThreads; ctx->info[2] = (int32_t)pl.smem;
     ctx->info[3] = rows_store; ctx->info[7] = pl.mode;

@@ -318,11 +318,10 @@ def test_error_codes_on_device_calls():
 
 # ------------------------------------------------------------------ every code path of the fill kernel
 @pytest.mark.parametrize("env", [{"HT_FILL_MODE": "0"},            # batch classification (global buckets) on single events too
-                                 {"HT_FILL_DYNAMIC": "1"},          # tiles handed out through the global counter
                                  {"HT_FILL_HIT_CAP": "32"},         # most hits bypass the shared-memory staging
                                  {"HT_FILL_SLAB_KB": "8"},          # many small tiles, rows shared by few warps
                                  {"HT_FILL_NO_BULK": "1"},          # plain stores instead of the TMA
-                                 {"HT_FILL_MODE": "0", "HT_FILL_DYNAMIC": "1", "HT_FILL_HIT_CAP": "0"}])
+                                 {"HT_FILL_MODE": "0", "HT_FILL_HIT_CAP": "0"}])
 def test_fill_kernel_variants_are_bit_exact(env, monkeypatch):
     """The launch-time switches of the fill kernel (read from the environment at every call) change how the work is
     organised, never the result."""
@@ -518,3 +517,52 @@ def test_plane_ranges_reassemble_the_full_result(world):
             B.ht_destroy(ctx)
     for parts in (parts_split, parts_fused):
         np.testing.assert_array_equal(sort_peaks(np.concatenate(parts), bn.cells), want_p)
+
+
+def test_calls_replayed_from_a_cuda_graph():
+    """The calls keep no host-side state between launches (barriers and counters reset themselves on the device), so a
+    captured sequence can be replayed: fill + peaks of two different events, three replays, results checked each time."""
+    wl = WORKLOADS[2]
+    bn = Binning(4, 16, 256, 256)
+    dev = torch.device("cuda:0")
+    batches = [generate_batch(wl, n_events=1, first_event=e) for e in range(2)]
+    wants = []
+    for b in batches:
+        m = _oracle_batch(bn, b)
+        wants.append((m[0], oracle_peaks_batch(bn, m, wl.threshold)))
+    cfg = B.ht_config.from_binning(bn, max_events=1, max_hits=max(b.n_hits for b in batches), device=0)
+    ctx = B.ht_create(cfg)
+    try:
+        to = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dev, dtype=dt)
+        ins = [(to(b.x, torch.float32), to(b.y, torch.float32), to(b.z, torch.float32), to(b.event_offsets, torch.int32))
+               for b in batches]
+        mhs = [torch.empty(bn.cells, dtype=torch.int32, device=dev) for _ in batches]
+        outs = [torch.zeros(3 << 13, dtype=torch.int32, device=dev) for _ in batches]
+        nfs = [torch.zeros(1, dtype=torch.int32, device=dev) for _ in batches]
+        st = torch.cuda.Stream()
+        def enqueue():
+            for k, b in enumerate(batches):
+                B.ht_fill_peaks(ctx, *ins[k], 1, b.n_hits, mhs[k], wl.threshold, outs[k], 1 << 13, nfs[k], st)
+        with torch.cuda.stream(st):
+            enqueue()                                              # warm-up outside the capture
+        st.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            enqueue()
+        for replay in range(3):
+            for k in range(2):
+                mhs[k].fill_(-1)
+                nfs[k].fill_(-5)
+            g.replay()
+            torch.cuda.synchronize()
+            for k in range(2):
+                want_m, want_p = wants[k]
+                np.testing.assert_array_equal(mhs[k].cpu().numpy().view(np.uint32), want_m.reshape(-1))
+                n = int(nfs[k].cpu().numpy().view(np.uint32)[0])
+                assert n == len(want_p)
+                rec = outs[k][:3 * n].cpu().numpy().view(np.uint32).reshape(n, 3)
+                pk = np.empty(n, B.PEAK_DTYPE)
+                pk["event"], pk["cell"], pk["count"] = rec[:, 0], rec[:, 1], rec[:, 2]
+                np.testing.assert_array_equal(sort_peaks(pk, bn.cells), want_p)
+    finally:
+        B.ht_destroy(ctx)
