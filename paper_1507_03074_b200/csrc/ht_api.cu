@@ -445,6 +445,7 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     HT_CUDA(cudaStreamIsCapturing(st, &cap));
     const bool one_shot = pl.mode == 1 && cap == cudaStreamCaptureStatusNone;
+    a.tile_counter = ctx->d_counters + 6;
     a.bar_count = one_shot ? ctx->d_counters + 5 : nullptr;
     a.bar_target = ctx->bar_epoch + (uint32_t)grid;
     {   // both prologues synchronise the grid: co-residency is guaranteed by a cooperative launch
