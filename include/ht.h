@@ -25,6 +25,8 @@
  *     synchronisation, no allocation.  Results are valid once the caller has synchronised the stream.
  *     Calls on one context must be stream-ordered with respect to each other (a context is not
  *     thread-safe and keeps per-call scratch); separate contexts are independent.
+ *     The enqueuing calls may be captured into a CUDA graph and replayed (nothing they do depends on host-side
+ *     state that a replay would miss; the fill kernel is launched cooperatively: one CTA per SM must be co-resident).
  *   - Every function returns HT_OK (0) or a negative ht_status; nothing aborts or throws.
  *     ht_strerror gives text; for HT_ERR_CUDA the text of the last CUDA error seen by this thread.
  */
