@@ -14,9 +14,11 @@
  *
  * Conventions
  *   - Pointers named d_* are DEVICE pointers (on cfg.device), h_* are HOST pointers.  The caller owns every
- *     buffer it passes; the library owns only the ht_ctx (host struct + small device workspace: the angle tables,
- *     a few counters, per-hit scratch of the classification (20 bytes per hit of cfg.max_hits, 8 bytes per
- *     (event, plane)); and, if cfg.host_slots > 0, staging buffers and host_slots vote matrices for ht_run_host).
+ *     buffer it passes.  The context's device workspace (the angle tables, a few counters, per-hit scratch of the
+ *     classification: 24 bytes per hit of cfg.max_hits, 8 bytes per (event, plane); and, if cfg.host_slots > 0, the
+ *     input mirror and host_slots vote matrices of the host calls) is either handed in by the caller
+ *     (ht_query_sizes -> allocate -> ht_create_ex: the library then allocates NOTHING on the device) or allocated by
+ *     ht_create itself (convenience form).  With cfg.host_slots > 0 the context also owns pinned HOST staging blocks.
  *   - Layout of a vote matrix (R15): uint32 M[event][itheta][iphi][ia][ib], ib fastest;
  *     cell = ((itheta*Nphi + iphi)*NA + ia)*NB + ib  (< 2^32 required).  d_mh must be 16-byte aligned.
  *     A context with a plane range (cfg.plane_count > 0) holds only its planes: M[event][plane - plane_begin][ia][ib].
@@ -24,9 +26,15 @@
  *     void*, e.g. torch.cuda.Stream().cuda_stream; NULL = the legacy default stream).  No host
  *     synchronisation, no allocation.  Results are valid once the caller has synchronised the stream.
  *     Calls on one context must be stream-ordered with respect to each other (a context is not
- *     thread-safe and keeps per-call scratch); separate contexts are independent.
+ *     thread-safe and keeps per-call scratch); separate contexts are independent.  When a call arrives on another
+ *     stream than the previous call of the context, the library itself orders the two with an event (outside graph
+ *     capture), so kernels of one context never run out of enqueue order.  The host calls (ht_run_host,
+ *     ht_submit_host) enqueue on a stream owned by the context and are ordered the same way.
+ *     The calls leave the caller's current device unchanged (they switch to cfg.device and back).
  *     The enqueuing calls may be captured into a CUDA graph and replayed (nothing they do depends on host-side
- *     state that a replay would miss; the fill kernel is launched cooperatively: one CTA per SM must be co-resident).
+ *     state that a replay would miss).  The fill kernel synchronises its grid: one CTA per SM must be co-resident,
+ *     which ht_create verifies with the occupancy calculator (ht_tuning.cooperative_launch = 1 makes the runtime
+ *     verify it at every launch instead).
  *   - Every function returns HT_OK (0) or a negative ht_status; nothing aborts or throws.
  *     ht_strerror gives text; for HT_ERR_CUDA the text of the last CUDA error seen by this thread.
  */
@@ -68,7 +76,8 @@ typedef struct ht_config {
     int32_t max_events;                /* largest n_events of one ht_fill / ht_peaks call, >= 1 */
     int32_t max_hits;                  /* largest n_hits_total of one ht_fill call, >= 1 */
     int32_t device;                    /* CUDA ordinal */
-    int32_t host_slots;                /* >= 0: vote matrices owned by the context for ht_run_host (0: that call is unavailable) */
+    int32_t host_slots;                /* >= 0: slots (input block, result block, vote matrix) of the host calls ht_run_host /
+                                          ht_submit_host; 0: those calls are unavailable */
     uint32_t host_peak_capacity;       /* peak-list capacity of the context's staging buffer for ht_run_host */
     /* Plane range of this context (f2; the sector split of PAPER.md:77 "four M_H(A,B,theta), each matrix processing the
      * data of a single phi sector"): the context fills and scans only the (theta,phi) planes
@@ -84,15 +93,37 @@ typedef struct ht_peak {
     uint32_t count; /* M_H value of the cell */
 } ht_peak;
 
-/* Sizes implied by a configuration: bytes of one event's matrix, and device bytes ht_create will allocate. */
-HT_API int ht_query_sizes(const ht_config *cfg, size_t *mh_bytes_per_event, size_t *ctx_device_bytes);
+/* How the work is organised on the device.  Nothing here ever changes a result (the parity tests run every
+ * variant); all zero = the defaults.  Read ONCE by ht_create_ex; the library reads no environment variable. */
+typedef struct ht_tuning {
+    int32_t fill_batch_classification; /* 1: classify through global buckets (the batch path) also for single events */
+    int32_t fill_slab_kb;              /* > 0: cap of one shared-memory slab in KB (0: as large as fits) */
+    int32_t fill_hit_cap;              /* > 0: hits of a tile staged in shared memory at most; -1: none (0: default) */
+    int32_t fill_plain_stores;         /* 1: tiles leave with plain stores instead of bulk (TMA) stores */
+    int32_t fill_shared_atomics;       /* 1: votes are shared-memory atomics (0: warp-private read-modify-write) */
+    int32_t cooperative_launch;        /* 1: cudaLaunchCooperativeKernel (0: ordinary launch, programmatic dependent
+                                          launch: the next call's prologue overlaps this call's tail) */
+    int32_t host_copy_input;           /* 1: ht_run_host / ht_submit_host copy the hits to the device (0: single events
+                                          are read by the kernel straight from the pinned block, zero-copy) */
+    int32_t peaks_unroll;              /* 2, 4 or 8 independent 16-byte loads per thread of the peak scan (0: 2) */
+    int32_t peaks_ctas_per_sm;         /* > 0: cap of the peak scan's resident CTAs per SM */
+    int32_t reserved[7];               /* must be zero */
+} ht_tuning;
 
-/* Host-only: the tables the library builds and uploads (SPEC.md section 1), for bit-for-bit comparison in tests.
- * two_a[n_a], t_theta[n_theta+1], p_phi[n_phi+1], d_ab[2] = {dA, dB}.  Needs no GPU. */
-HT_API int ht_tables_host(const ht_config *cfg, float *two_a, float *t_theta, float *p_phi, float *d_ab);
+/* Sizes implied by a configuration: bytes of one event's matrix, and bytes of the context's device workspace
+ * (what ht_create allocates, or what the caller hands to ht_create_ex). */
+HT_API int ht_query_sizes(const ht_config *cfg, size_t *mh_bytes_per_event, size_t *workspace_bytes);
 
-/* Validate cfg, build and upload tables, allocate the workspace on cfg.device.  *out is set only on HT_OK. */
+/* Validate cfg, build and upload the tables (SPEC.md section 1), allocate the workspace on cfg.device.
+ * *out is set only on HT_OK.  Same as ht_create_ex(cfg, NULL, NULL, 0, out).  (Defines no step of the method.) */
 HT_API int ht_create(const ht_config *cfg, ht_ctx **out);
+
+/* ht_create with tuning switches (NULL: defaults) and a CALLER-OWNED device workspace: d_workspace (256-byte aligned,
+ * on cfg.device) of at least ht_query_sizes()'s workspace_bytes, which must outlive the context and is not freed by
+ * ht_destroy; the library then allocates no device memory at all.  d_workspace == NULL: the library allocates (and
+ * ht_destroy frees) the workspace.  HT_ERR_INVALID_ARG if the workspace is too small or misaligned. */
+HT_API int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning_or_null, void *d_workspace_or_null,
+                        size_t workspace_bytes, ht_ctx **out);
 
 /*
  * Fill the vote matrices of a batch of events (SPEC.md section 2).
@@ -164,34 +195,38 @@ typedef struct ht_track {
 HT_API int ht_tracks(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, ht_track *d_out, void *cuda_stream);
 
 /*
- * End-to-end call with HOST buffers (needs cfg.host_slots >= 1): packs offsets and hits into one pinned block, which
- * the kernel reads directly (one event: every hit is read exactly once, zero-copy over PCIe) or which is copied to the
- * device in one transfer (batches), runs ht_fill_peaks (or ht_fill + ht_peaks where that is unsupported) on the
- * context's own matrices (events in groups of host_slots) with the peak list and count written by the kernel straight
- * into mapped pinned memory, and synchronises.  h_out receives min(*h_n_found, capacity) records;
- * capacity <= cfg.host_peak_capacity.
+ * End-to-end call with HOST buffers (f4; needs cfg.host_slots >= 1; the transfer is "the dominant part" of
+ * the paper's total time -- here only the hits (12 bytes each) and the compacted peak list cross PCIe).
+ * Packs offsets and hits into one pinned block, which the kernel reads directly (one event: every hit is read exactly
+ * once, zero-copy over PCIe) or which is copied to the device in one transfer (batches, ht_tuning.host_copy_input),
+ * runs ht_fill_peaks (or ht_fill + ht_peaks where that is unsupported) on the context's own matrices (events in groups
+ * of host_slots) with the peak list and count written by the kernel straight into mapped pinned memory, and
+ * synchronises.  h_out receives min(*h_n_found, capacity) records; capacity <= cfg.host_peak_capacity.
  * h_mh_or_null: if not NULL, n_events * cells uint32 that also receive the matrices (testing; slow).
- * Host buffers may be pageable or pinned (pinned makes the copies asynchronous DMA).
+ * Host buffers may be pageable or pinned.  No event may be in flight in a slot (ht_submit_host without ht_wait_host).
  */
 HT_API int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_z,
                        const int32_t *h_event_offsets, int32_t n_events, int32_t n_hits_total, uint32_t threshold,
                        ht_peak *h_out, uint32_t capacity, uint32_t *h_n_found, uint32_t *h_mh_or_null);
 
-/* Number of kernels this context has launched so far (host-side counter; for bench.py's gpu_launches). */
-HT_API int64_t ht_kernel_launches(const ht_ctx *ctx);
+/*
+ * The same end-to-end path, asynchronous, one event per call, so that packing event k+1 and reading the peaks of event
+ * k-1 overlap the kernel of event k:
+ *   ht_submit_host  copies the n_hits hits of ONE event from h_x, h_y, h_z into the pinned input block of `slot`
+ *                   (0 <= slot < cfg.host_slots; the caller's arrays may be reused as soon as the call returns),
+ *                   enqueues the fused kernel (a0-a5; the event's matrix is materialised in the slot's own matrix) on the
+ *                   context's stream and returns without waiting.  HT_ERR_INVALID_ARG if the slot still holds an event
+ *                   that has not been waited for.  Events run in submission order.
+ *   ht_wait_host    blocks until the event submitted into `slot` has finished; h_out receives
+ *                   min(*h_n_found, capacity, cfg.host_peak_capacity) records, *h_n_found the number of peaks found.
+ *                   HT_ERR_INVALID_ARG if nothing was submitted into the slot.
+ * ht_run_host on one event is ht_submit_host + ht_wait_host on slot 0.
+ */
+HT_API int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y, const float *h_z, int32_t n_hits,
+                          uint32_t threshold);
+HT_API int ht_wait_host(ht_ctx *ctx, int32_t slot, ht_peak *h_out, uint32_t capacity, uint32_t *h_n_found);
 
-/* Launch geometry of the last ht_fill / ht_peaks (for DESIGN.md / bench reporting): out[0]=fill grid, out[1]=fill block,
- * out[2]=fill dynamic smem bytes, out[3]=rows stored per tile, out[4]=peaks grid, out[5]=peaks block, out[6]=SM count,
- * out[7]=classification mode of the last fill (1: one event, hit index in shared memory; 0: batch, buckets in global memory). */
-HT_API int ht_launch_info(const ht_ctx *ctx, int32_t out[8]);
-
-/* Self-test of the arithmetic shortcut of the vote loop ("Exact division"): evaluates n_pairs
- * pseudo-random quotients a/b (all significand patterns, exponents across and just outside the range the shortcut is
- * used on) both ways on `device` and returns in *h_mismatches how many differ in any bit from __fdiv_rn (must be 0).
- * Synchronous; allocates and frees 8 bytes of device memory. */
-HT_API int ht_selftest_division(int32_t device, uint64_t n_pairs, uint64_t seed, uint64_t *h_mismatches);
-
-/* Free everything the context owns.  NULL is allowed. */
+/* Free everything the context owns (not a caller-owned workspace).  NULL is allowed.  (Defines no step of the method.) */
 HT_API void ht_destroy(ht_ctx *ctx);
 
 HT_API const char *ht_strerror(int status);

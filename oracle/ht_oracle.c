@@ -23,9 +23,11 @@
  * cell-centric brute force in double with atan2 binning on tiny binnings (P4), single-hit geometry (P5),
  * mirror symmetry (P6), permutation/batching invariance (P7), hand-built peak matrices (P8),
  * peak-set invariants (P9), table binning vs atan2 (P10), closed-form in-range fraction; track read-out: the
- * truth circle of a noiseless track (P11), polar identities and special cells (P12).
+ * truth circle of a noiseless track (P11), polar identities and special cells (P12); ridge merging: connected-component
+ * labelling of a library routine on a doubled grid (P13), hand-built peak layouts (P14), partition invariants (P15).
  * Parity unpinned by the paper (definitions fixed by SPEC.md only): R2/R4 angle definition and
- * ranges, R5 bin centre, R10 neighbourhood, R11 >= vs >, R12 tie rule, R17 quadrant of phi.
+ * ranges, R5 bin centre, R10 neighbourhood, R11 >= vs >, R12 tie rule, R17 quadrant of phi, R19 (the merge rule itself
+ * is this build's stand-in for the paper's unexplained step from local maxima to tracks).
  */
 #include <math.h>
 #include <stdint.h>
@@ -269,4 +271,81 @@ int oracle_tracks(const oracle_binning *g, const oracle_peak *peaks, int64_t n, 
         phi[k] = atan2((double)B, (double)A);
     }
     return 0;
+}
+
+/*
+ * Ridge merging of a peak list (SPEC.md section 5, reading R19; SURVEY.md section 8(f) f3 "merging ridge peaks").
+ * PAPER.md:25 goes from "local maxima" straight to "real tracks"; a stiff track's vote lines are nearly parallel, so its
+ * maximum is a RIDGE on which several non-adjacent cells pass the peak rule.  R19: two peaks of the same event and the
+ * same (theta,phi) plane are LINKED when their cells are at Chebyshev distance <= window in (a, b); a track candidate is
+ * a connected component of the link graph; its representative is the member with the largest count, the smallest cell
+ * among equals.  out[k] = (event, representative cell, its count, members, rho, phi of the representative as in
+ * oracle_tracks), sorted by (event, cell).  Plain definition: every pair is tested, textbook union-find.
+ * Returns the number of components (-1 on bad arguments); writes at most `capacity`.
+ */
+typedef struct { uint32_t event, cell, count, n_peaks; double rho, phi; } oracle_merged;
+
+static int64_t uf_find(int64_t *parent, int64_t i)
+{
+    while (parent[i] != i) i = parent[i];
+    return i;
+}
+
+static int merged_less(const oracle_merged *a, const oracle_merged *b)
+{
+    return a->event < b->event || (a->event == b->event && a->cell < b->cell);
+}
+
+int64_t oracle_merge_ridges(const oracle_binning *g, const oracle_peak *peaks, int64_t n, uint32_t window,
+                            oracle_merged *out, int64_t capacity)
+{
+    if (!binning_ok(g) || n < 0 || capacity < 0 || (n > 0 && !peaks)) return -1;
+    const int64_t NA = g->n_a, NB = g->n_b;
+    const uint64_t cells = (uint64_t)g->n_theta * g->n_phi * g->n_a * g->n_b;
+    for (int64_t i = 0; i < n; ++i)
+        if (peaks[i].cell >= cells) return -1;
+    int64_t *parent = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n + 1));
+    if (!parent) return -1;
+    for (int64_t i = 0; i < n; ++i) parent[i] = i;
+    for (int64_t i = 0; i < n; ++i) {
+        const int64_t bi = peaks[i].cell % NB, ai = (peaks[i].cell / NB) % NA, pi = peaks[i].cell / (NB * NA);
+        for (int64_t j = i + 1; j < n; ++j) {
+            if (peaks[j].event != peaks[i].event) continue;
+            const int64_t bj = peaks[j].cell % NB, aj = (peaks[j].cell / NB) % NA, pj = peaks[j].cell / (NB * NA);
+            if (pj != pi) continue;                                  /* never across (theta,phi) planes (R10) */
+            const int64_t da = ai > aj ? ai - aj : aj - ai, db = bi > bj ? bi - bj : bj - bi;
+            if ((da > db ? da : db) > (int64_t)window) continue;    /* Chebyshev distance */
+            const int64_t ri = uf_find(parent, i), rj = uf_find(parent, j);
+            if (ri != rj) parent[ri] = rj;
+        }
+    }
+    int64_t found = 0;
+    oracle_merged *all = (oracle_merged *)malloc(sizeof(oracle_merged) * (size_t)(n + 1));
+    if (!all) { free(parent); return -1; }
+    for (int64_t r = 0; r < n; ++r) {
+        if (parent[r] != r) continue;                                /* one component per root */
+        int64_t best = -1;
+        uint32_t members = 0;
+        for (int64_t i = 0; i < n; ++i) {
+            if (uf_find(parent, i) != r) continue;
+            ++members;
+            if (best < 0 || peaks[i].count > peaks[best].count ||
+                (peaks[i].count == peaks[best].count && peaks[i].cell < peaks[best].cell)) best = i;
+        }
+        oracle_merged m;
+        m.event = peaks[best].event; m.cell = peaks[best].cell; m.count = peaks[best].count; m.n_peaks = members;
+        oracle_peak one = peaks[best];
+        if (oracle_tracks(g, &one, 1, &m.rho, &m.phi) != 0) { free(parent); free(all); return -1; }
+        all[found++] = m;
+    }
+    for (int64_t i = 1; i < found; ++i) {                            /* insertion sort by (event, cell) */
+        oracle_merged key = all[i];
+        int64_t j = i - 1;
+        while (j >= 0 && merged_less(&key, &all[j])) { all[j + 1] = all[j]; --j; }
+        all[j + 1] = key;
+    }
+    for (int64_t i = 0; i < found && i < capacity; ++i) out[i] = all[i];
+    free(parent);
+    free(all);
+    return found;
 }

@@ -11,6 +11,8 @@ import numpy as np
 from .build import build
 
 PEAK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32)])
+MERGED_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32), ("n_peaks", np.uint32),
+                         ("rho", np.float64), ("phi", np.float64)])                       # == oracle_merged
 
 
 class OracleBinning(C.Structure):
@@ -55,6 +57,9 @@ def _load():
         lib.oracle_tracks.restype = C.c_int
         lib.oracle_tracks.argtypes = [C.POINTER(OracleBinning), C.c_void_p, C.c_int64, C.POINTER(C.c_double),
                                       C.POINTER(C.c_double)]
+        lib.oracle_merge_ridges.restype = C.c_int64
+        lib.oracle_merge_ridges.argtypes = [C.POINTER(OracleBinning), C.c_void_p, C.c_int64, C.c_uint32, C.c_void_p,
+                                            C.c_int64]
         _lib = lib
     return _lib
 
@@ -156,3 +161,15 @@ def oracle_tracks(binning, peaks: np.ndarray):
                              phi.ctypes.data_as(dp)) != 0:
         raise ValueError("oracle_tracks: invalid arguments (cell outside the matrix?)")
     return rho, phi
+
+
+def oracle_merge_ridges(binning, peaks: np.ndarray, window: int) -> np.ndarray:
+    """Track candidates of a peak list (SPEC.md section 5, R19): MERGED_DTYPE records sorted by (event, cell)."""
+    g = OracleBinning.of(binning)
+    pk = np.ascontiguousarray(peaks, dtype=PEAK_DTYPE)
+    out = np.empty(len(pk), MERGED_DTYPE)
+    n = _load().oracle_merge_ridges(C.byref(g), pk.ctypes.data_as(C.c_void_p), len(pk), window,
+                                    out.ctypes.data_as(C.c_void_p), len(pk))
+    if n < 0:
+        raise ValueError("oracle_merge_ridges: invalid arguments")
+    return out[:n]

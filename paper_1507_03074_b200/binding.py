@@ -21,8 +21,12 @@ PEAK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.u
 TRACK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32),
                         ("rho", np.float32), ("phi", np.float32)])                                # == struct ht_track
 
-EXPORTS = ("ht_query_sizes", "ht_tables_host", "ht_create", "ht_fill", "ht_fill_peaks", "ht_fill_naive", "ht_peaks", "ht_tracks", "ht_run_host",
-           "ht_selftest_division", "ht_kernel_launches", "ht_launch_info", "ht_destroy", "ht_strerror")
+EXPORTS = ("ht_query_sizes", "ht_create", "ht_create_ex", "ht_fill", "ht_fill_peaks", "ht_fill_naive", "ht_peaks", "ht_tracks",
+           "ht_run_host", "ht_submit_host", "ht_wait_host", "ht_destroy", "ht_strerror")                  # include/ht.h
+DIAG_EXPORTS = ("ht_tables_host", "ht_kernel_launches", "ht_launch_info", "ht_selftest_division", "ht_diag_memset",
+                "ht_diag_vote_rates")                                                                     # include/ht_diag.h
+DIAG_PATTERNS = ("red_random", "red_random_71", "red_no_conflict", "red_two_way", "red_same", "atom_random",
+                 "atom_no_conflict", "atom_same", "rmw_random_inexact", "tag_random", "match_random", "tag_random_71")
 
 
 class ht_config(C.Structure):
@@ -45,6 +49,14 @@ class ht_config(C.Structure):
         """Cells of one event's matrix IN THIS CONTEXT (its plane range only)."""
         planes = self.plane_count if self.plane_count > 0 else self.n_theta * self.n_phi
         return planes * self.n_a * self.n_b
+
+
+class ht_tuning(C.Structure):
+    """How the work is organised on the device (include/ht.h); never changes a result.  All zero = defaults."""
+    _fields_ = [("fill_batch_classification", C.c_int32), ("fill_slab_kb", C.c_int32), ("fill_hit_cap", C.c_int32),
+                ("fill_plain_stores", C.c_int32), ("fill_shared_atomics", C.c_int32), ("cooperative_launch", C.c_int32),
+                ("host_copy_input", C.c_int32), ("peaks_unroll", C.c_int32), ("peaks_ctas_per_sm", C.c_int32),
+                ("reserved", C.c_int32 * 7)]
 
 
 class HtError(RuntimeError):
@@ -73,6 +85,16 @@ def load() -> C.CDLL:
     lib.ht_tables_host.argtypes = [cfgp, vp, vp, vp, vp]
     lib.ht_create.restype = C.c_int
     lib.ht_create.argtypes = [cfgp, C.POINTER(vp)]
+    lib.ht_create_ex.restype = C.c_int
+    lib.ht_create_ex.argtypes = [cfgp, C.POINTER(ht_tuning), vp, C.c_size_t, C.POINTER(vp)]
+    lib.ht_submit_host.restype = C.c_int
+    lib.ht_submit_host.argtypes = [vp, i32, vp, vp, vp, i32, u32]
+    lib.ht_wait_host.restype = C.c_int
+    lib.ht_wait_host.argtypes = [vp, i32, vp, u32, vp]
+    lib.ht_diag_memset.restype = C.c_int
+    lib.ht_diag_memset.argtypes = [vp, i32, C.c_size_t, vp]
+    lib.ht_diag_vote_rates.restype = C.c_int
+    lib.ht_diag_vote_rates.argtypes = [i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
     for name in ("ht_fill", "ht_fill_naive"):
         fn = getattr(lib, name)
         fn.restype = C.c_int
@@ -151,6 +173,15 @@ def ht_create(cfg: ht_config) -> int:
     return out.value
 
 
+def ht_create_ex(cfg: ht_config, tuning: ht_tuning | None = None, d_workspace=None, workspace_bytes: int = 0) -> int:
+    """ht_create with tuning switches and/or a caller-owned device workspace (a tensor or an address) of at least
+    ``ht_query_sizes(cfg)[1]`` bytes, 256-byte aligned, which must outlive the context."""
+    out = C.c_void_p()
+    _check(load().ht_create_ex(C.byref(cfg), C.byref(tuning) if tuning is not None else None, _ptr(d_workspace),
+                               workspace_bytes, C.byref(out)), "ht_create_ex")
+    return out.value
+
+
 def ht_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events: int, n_hits_total: int, d_mh, stream=None) -> None:
     _check(load().ht_fill(ctx, _ptr(d_x), _ptr(d_y), _ptr(d_z), _ptr(d_event_offsets), n_events, n_hits_total,
                           _ptr(d_mh), _stream(stream)), "ht_fill")
@@ -187,6 +218,30 @@ def ht_run_host(ctx, h_x, h_y, h_z, h_event_offsets, n_events: int, n_hits_total
     _check(load().ht_run_host(ctx, _ptr(h_x), _ptr(h_y), _ptr(h_z), _ptr(h_event_offsets), n_events, n_hits_total,
                               threshold, _ptr(h_out), capacity, C.addressof(n), _ptr(h_mh)), "ht_run_host")
     return n.value
+
+
+def ht_submit_host(ctx, slot: int, h_x, h_y, h_z, n_hits: int, threshold: int) -> None:
+    """Asynchronous half of the end-to-end call: ONE event from host buffers into slot ``slot`` (returns at once)."""
+    _check(load().ht_submit_host(ctx, slot, _ptr(h_x), _ptr(h_y), _ptr(h_z), n_hits, threshold), "ht_submit_host")
+
+
+def ht_wait_host(ctx, slot: int, h_out, capacity: int) -> int:
+    """Waits for the event submitted into ``slot``; ``h_out`` receives min(found, capacity) records.  Returns found."""
+    n = C.c_uint32(0)
+    _check(load().ht_wait_host(ctx, slot, _ptr(h_out), capacity, C.addressof(n)), "ht_wait_host")
+    return n.value
+
+
+def ht_diag_memset(d_dst, value: int, nbytes: int, stream=None) -> None:
+    _check(load().ht_diag_memset(_ptr(d_dst), value, nbytes, _stream(stream)), "ht_diag_memset")
+
+
+def ht_diag_vote_rates(device: int = 0, iters: int = 2000) -> tuple[dict, int]:
+    """({pattern: votes per clock per SM}, rows whose sum was wrong) -- the shared-memory vote micro-benchmark."""
+    rates = (C.c_double * len(DIAG_PATTERNS))()
+    err = C.c_uint64(0)
+    _check(load().ht_diag_vote_rates(device, iters, rates, C.byref(err)), "ht_diag_vote_rates")
+    return dict(zip(DIAG_PATTERNS, list(rates))), int(err.value)
 
 
 def ht_selftest_division(device: int, n_pairs: int, seed: int) -> int:

@@ -10,7 +10,8 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libht.so")
 SOURCES = [os.path.join(CSRC, "ht_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "ht_device.cuh"), os.path.join(INCLUDE, "ht.h")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("ht_device.cuh", "ht_diag.cuh", "ht_merge.cuh")] + \
+       [os.path.join(INCLUDE, f) for f in ("ht.h", "ht_diag.h")]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -31,7 +32,7 @@ def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(d) > t for d in DEPS)
+    return any(os.path.exists(d) and os.path.getmtime(d) > t for d in DEPS)
 
 
 def build(force: bool = False, verbose: bool = False, extra: list[str] | None = None) -> str:

@@ -1,8 +1,12 @@
-// ht_api.cu -- C ABI of libht (include/ht.h): argument validation, table construction (SPEC.md section 1),
-// workspace management and kernel launches.  No torch types, no exceptions across the boundary.
+// ht_api.cu -- C ABI of libht (include/ht.h, include/ht_diag.h): argument validation, table construction (SPEC.md
+// section 1), workspace layout and kernel launches.  No torch types, no exceptions across the boundary, no environment
+// variables: every switch is a field of ht_tuning, read once by ht_create_ex.
 #include "../../include/ht.h"
+#include "../../include/ht_diag.h"
 #include "ht_device.cuh"
+#include "ht_diag.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -28,12 +32,24 @@ int cuda_fail(cudaError_t e, const char *what)
 
 constexpr double kPi = 3.14159265358979323846;
 
-int env_int(const char *name, int dflt)
-{
-    const char *s = std::getenv(name);
-    if (!s || !*s) return dflt;
-    return std::atoi(s);
-}
+// The calls leave the caller's current device as they found it.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int dev)
+    {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != dev) {
+            err = cudaSetDevice(dev);
+            switched = err == cudaSuccess;
+        }
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 
 bool config_ok(const ht_config *c)
 {
@@ -54,6 +70,11 @@ bool config_ok(const ht_config *c)
     if (c->plane_count > 0 && (long long)c->plane_begin + c->plane_count > (long long)c->n_theta * c->n_phi) return false;
     if (c->plane_count == 0 && c->plane_begin != 0) return false;
     return true;
+}
+
+bool sizes_ok(const ht_config *c)
+{
+    return config_ok(c) && c->max_events >= 1 && c->max_hits >= 1 && c->host_slots >= 0 && c->max_hits <= INT32_MAX - 65536;
 }
 
 double cot(double t) { return std::cos(t) / std::sin(t); }
@@ -95,14 +116,69 @@ void build_tables(const ht_config *c, float *two_a, float *tth, float *pph, floa
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+constexpr size_t kResHeader = 16;      // result block: [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
+
+// Layout of the context's device workspace (one contiguous block: caller-owned or allocated by ht_create) and sizes of
+// the pinned host staging blocks.  Offsets are multiples of 256.
+struct WorkspaceLayout {
+    size_t tables, counters, hits, bucket_start, counts, in_dev, mh;      // offsets
+    size_t hits_part;             // bytes of one of the 6 per-hit arrays
+    size_t in_block, res_block;   // bytes of ONE slot's input block [offsets | x | y | z] and result block
+    size_t total;
+};
+
+WorkspaceLayout workspace_layout(const ht_config *c)
+{
+    WorkspaceLayout w{};
+    const size_t planes_all = (size_t)c->n_theta * (size_t)c->n_phi;
+    const size_t cells = (c->plane_count > 0 ? (size_t)c->plane_count : planes_all) * (size_t)c->n_a * (size_t)c->n_b;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += align_up(bytes, 256); return o; };
+    w.tables = take(sizeof(float) * (size_t)(c->n_theta + 1 + c->n_phi + 1));
+    w.counters = take(256);
+    w.hits_part = align_up(sizeof(float) * (size_t)c->max_hits, 256);
+    w.hits = take(6 * w.hits_part);            // hit records (4 words per hit), h_plane, h_rel
+    w.bucket_start = take(sizeof(int32_t) * (size_t)c->max_events * (planes_all + 1));
+    w.counts = take(sizeof(uint32_t) * (size_t)c->max_events * planes_all);
+    if (c->host_slots > 0) {
+        w.in_block = align_up(align_up(sizeof(int32_t) * ((size_t)c->max_events + 1), 16) +
+                              3 * align_up(sizeof(float) * (size_t)c->max_hits, 16), 256);
+        w.res_block = align_up(kResHeader + sizeof(ht_peak) * (size_t)c->host_peak_capacity, 256);
+        w.in_dev = take(w.in_block * (size_t)c->host_slots);
+        w.mh = take(cells * sizeof(uint32_t) * (size_t)c->host_slots);
+    }
+    w.total = off;
+    return w;
+}
+
+// Tile geometry of the fill kernel for one call: the largest slab (rows of NB cells) such that two slabs, the row
+// tables, the staged hits and -- in mode 1 -- the plane offsets and the uint16 hit index fit the CTA's shared memory.
+struct FillPlan {
+    bool ok = false;
+    int mode = 0, rows_slab = 0, hit_cap = 0;
+    uint32_t slab_words = 0;
+    size_t smem = 0;
+};
+
+struct HostSlot {
+    unsigned char *h_in = nullptr, *d_in = nullptr, *d_in_mapped = nullptr;   // pinned input block, its device mirror, its device alias
+    unsigned char *h_res = nullptr, *d_res = nullptr;                          // mapped pinned result block and its device alias
+    cudaEvent_t copied = nullptr, done = nullptr;
+    bool busy = false;
+};
+
 }  // namespace
 
 struct ht_ctx {
     ht_config cfg;
+    ht_tuning tun;
     ht::Geom geom;
     int sm_count = 0;
     int max_smem_optin = 0;
     // device workspace
+    unsigned char *d_ws = nullptr;
+    bool owns_ws = false;
+    WorkspaceLayout lay{};
     float *d_tth = nullptr, *d_pph = nullptr;
     uint32_t *d_counters = nullptr;
     // hit buckets written by the fill kernel's prologue (a0): per-hit vote constants grouped by (event, plane)
@@ -110,61 +186,27 @@ struct ht_ctx {
     int32_t *d_hplane = nullptr, *d_hrel = nullptr;   // [max_hits] phase-1 spill
     int32_t *d_bucket_start = nullptr;     // [max_events * (P+1)]
     uint32_t *d_counts = nullptr;          // [max_events * P], zero between calls
-    // tile fill launch geometry: per-kernel dynamic shared memory budget ([0]: ht_fill, [1]: fused peaks), and whether
-    // the device can run the kernel at all (one CTA of 1024 threads per SM, cooperative launch for mode 0)
-    uint32_t bar_epoch = 0;                   // host mirror of the barrier counter that only grows (d_counters[5])
+    uint32_t bar_epoch = 0;                // host mirror of the barrier counter that only grows (d_counters[5])
     bool fill_ok = false;
-    size_t fill_smem_max[2] = {0, 0};
+    size_t fill_smem_max[2] = {0, 0};      // dynamic shared memory budget: [0] ht_fill, [1] fused peaks
+    FillPlan plan_cache[2];
+    int plan_key[2][2] = {{-1, -1}, {-1, -1}};      // (n_events, n_hits) of plan_cache[peaks]
     // peak scan launch geometry
-    int peaks_unroll = 4, peaks_grid_vec4 = 0, peaks_grid_vec1 = 0;
-    // host path (ht_run_host)
-    unsigned char *d_in = nullptr;     // [offsets | x | y | z], packed per call (one H2D copy)
-    unsigned char *h_in = nullptr;     // pinned + mapped mirror of d_in
-    unsigned char *d_in_mapped = nullptr;   // device alias of h_in (zero-copy input of single events)
+    int peaks_unroll = 2, peaks_grid_vec4 = 0, peaks_grid_vec1 = 0;
+    // stream ordering between calls of this context
+    cudaStream_t last_stream = nullptr;
+    bool has_last = false;
+    cudaEvent_t order_event = nullptr;
+    // host path (ht_run_host, ht_submit_host / ht_wait_host)
+    unsigned char *h_in_all = nullptr, *h_res_all = nullptr;
+    std::vector<HostSlot> slots;
     uint32_t *d_hmh = nullptr;
-    unsigned char *h_res = nullptr;    // pinned + mapped: [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
-    unsigned char *d_res = nullptr;    // device alias of h_res: the kernels write the peak list straight to the host
-    cudaStream_t host_stream = nullptr;
+    cudaStream_t host_stream = nullptr, copy_stream = nullptr;
     int64_t launches = 0;
     int32_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 };
 
 namespace {
-
-constexpr size_t kResHeader = 16;
-
-struct WorkspaceSizes {
-    size_t tables, counters, buckets, bucket_start, counts, host_hits, host_off, host_mh, host_res, total;
-};
-
-WorkspaceSizes workspace_sizes(const ht_config *c)
-{
-    WorkspaceSizes w{};
-    const size_t planes = (size_t)c->n_theta * (size_t)c->n_phi;
-    const size_t cells = (c->plane_count > 0 ? (size_t)c->plane_count : planes) * (size_t)c->n_a * (size_t)c->n_b;
-    w.tables = align_up(sizeof(float) * (size_t)(c->n_theta + 1 + c->n_phi + 1), 256);
-    w.counters = 256;
-    w.buckets = 6 * align_up(sizeof(float) * (size_t)c->max_hits, 256);      // hit records (4 words per hit), h_plane, h_rel
-    w.bucket_start = align_up(sizeof(int32_t) * (size_t)c->max_events * (planes + 1), 256);
-    w.counts = align_up(sizeof(uint32_t) * (size_t)c->max_events * planes, 256);
-    if (c->host_slots > 0) {
-        w.host_hits = 3 * align_up(sizeof(float) * (size_t)c->max_hits, 16);
-        w.host_off = align_up(sizeof(int32_t) * ((size_t)c->max_events + 1), 16);
-        w.host_mh = align_up(cells * sizeof(uint32_t) * (size_t)c->host_slots, 256);
-        w.host_res = align_up(kResHeader + sizeof(ht_peak) * (size_t)c->host_peak_capacity, 256);
-    }
-    w.total = w.tables + w.counters + w.buckets + w.bucket_start + w.counts + w.host_hits + w.host_off + w.host_mh;
-    return w;
-}
-
-// Tile geometry of the fill kernel for one call: the largest slab (rows of NB cells) such that four slabs (two per warp
-// group), the row tables, and -- in mode 1 -- the plane offsets and the uint16 hit index fit the CTA's shared memory.
-struct FillPlan {
-    bool ok = false;
-    int mode = 0, rows_slab = 0, hit_cap = 0;
-    uint32_t slab_words = 0;
-    size_t smem = 0;
-};
 
 size_t fill_smem_bytes(const ht_config &c, long long rows, int mode, long long n_hits)
 {
@@ -188,17 +230,35 @@ int check_fill_args(ht_ctx *ctx, const float *d_x, const float *d_y, const float
     return HT_OK;
 }
 
+// Kernels of one context share its scratch, so they must run in enqueue order.  A call that arrives on another stream
+// than the previous one is ordered behind it with an event (not during graph capture: there the caller's capture
+// dependencies are what they are).
+int order_after_previous(ht_ctx *ctx, cudaStream_t st)
+{
+    if (ctx->has_last && ctx->last_stream != st) {
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        HT_CUDA(cudaStreamIsCapturing(st, &cap));
+        if (cap == cudaStreamCaptureStatusNone) {
+            HT_CUDA(cudaEventRecord(ctx->order_event, ctx->last_stream));
+            HT_CUDA(cudaStreamWaitEvent(st, ctx->order_event, 0));
+        }
+    }
+    ctx->last_stream = st;
+    ctx->has_last = true;
+    return HT_OK;
+}
+
 }  // namespace
 
 extern "C" {
 
-int ht_query_sizes(const ht_config *cfg, size_t *mh_bytes_per_event, size_t *ctx_device_bytes)
+int ht_query_sizes(const ht_config *cfg, size_t *mh_bytes_per_event, size_t *workspace_bytes)
 {
-    if (!config_ok(cfg) || cfg->max_events < 1 || cfg->max_hits < 1 || cfg->host_slots < 0) return HT_ERR_INVALID_ARG;
+    if (!sizes_ok(cfg)) return HT_ERR_INVALID_ARG;
     const size_t planes = cfg->plane_count > 0 ? (size_t)cfg->plane_count : (size_t)cfg->n_theta * (size_t)cfg->n_phi;
     const size_t cells = planes * (size_t)cfg->n_a * (size_t)cfg->n_b;
     if (mh_bytes_per_event) *mh_bytes_per_event = cells * sizeof(uint32_t);
-    if (ctx_device_bytes) *ctx_device_bytes = workspace_sizes(cfg).total;
+    if (workspace_bytes) *workspace_bytes = workspace_layout(cfg).total;
     return HT_OK;
 }
 
@@ -209,19 +269,33 @@ int ht_tables_host(const ht_config *cfg, float *two_a, float *t_theta, float *p_
     return HT_OK;
 }
 
-int ht_create(const ht_config *cfg, ht_ctx **out)
+int ht_create(const ht_config *cfg, ht_ctx **out) { return ht_create_ex(cfg, nullptr, nullptr, 0, out); }
+
+int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspace, size_t workspace_bytes, ht_ctx **out)
 {
     if (!out) return HT_ERR_INVALID_ARG;
-    if (!config_ok(cfg) || cfg->max_events < 1 || cfg->max_hits < 1 || cfg->host_slots < 0) return HT_ERR_INVALID_ARG;
-    if (cfg->max_hits > INT32_MAX - 65536) return HT_ERR_INVALID_ARG;
+    if (!sizes_ok(cfg)) return HT_ERR_INVALID_ARG;
+    ht_tuning tun{};
+    if (tuning) {
+        tun = *tuning;
+        for (int32_t r : tun.reserved)
+            if (r != 0) return HT_ERR_INVALID_ARG;
+        if (tun.peaks_unroll != 0 && tun.peaks_unroll != 2 && tun.peaks_unroll != 4 && tun.peaks_unroll != 8) return HT_ERR_INVALID_ARG;
+        if (tun.fill_slab_kb < 0 || tun.fill_hit_cap < -1 || tun.peaks_ctas_per_sm < 0) return HT_ERR_INVALID_ARG;
+    }
+    const WorkspaceLayout lay = workspace_layout(cfg);
+    if (d_workspace && (workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0)) return HT_ERR_INVALID_ARG;
     int ndev = 0;
     HT_CUDA(cudaGetDeviceCount(&ndev));
     if (cfg->device < 0 || cfg->device >= ndev) return HT_ERR_INVALID_ARG;
-    HT_CUDA(cudaSetDevice(cfg->device));
+    DeviceGuard guard(cfg->device);
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "cudaSetDevice");
 
     ht_ctx *ctx = new (std::nothrow) ht_ctx();
     if (!ctx) return HT_ERR_NOMEM;
     ctx->cfg = *cfg;
+    ctx->tun = tun;
+    ctx->lay = lay;
     ht::Geom &g = ctx->geom;
     g.n_theta = cfg->n_theta; g.n_phi = cfg->n_phi; g.n_a = cfg->n_a; g.n_b = cfg->n_b;
     g.planes = cfg->plane_count > 0 ? cfg->plane_count : cfg->n_theta * cfg->n_phi;
@@ -234,56 +308,64 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     g.a_min = cfg->a_min; g.dA = d_ab[0]; g.b_min = cfg->b_min; g.dB = d_ab[1]; g.nb_f = (float)cfg->n_b;
 
     cudaError_t e;
-    int rc = HT_OK;
     auto fail = [&](int code) { ht_destroy(ctx); return code; };
     if ((e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, cfg->device)) != cudaSuccess)
         return fail(cuda_fail(e, "cudaDeviceGetAttribute(SM count)"));
     if ((e = cudaDeviceGetAttribute(&ctx->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device)) != cudaSuccess)
         return fail(cuda_fail(e, "cudaDeviceGetAttribute(smem optin)"));
 
-    const WorkspaceSizes w = workspace_sizes(cfg);
-    auto dmalloc = [&](void **p, size_t bytes, const char *what) -> bool {
-        if (bytes == 0) { *p = nullptr; return true; }
-        cudaError_t err = cudaMalloc(p, bytes);
-        if (err != cudaSuccess) {
-            rc = (err == cudaErrorMemoryAllocation) ? HT_ERR_NOMEM : cuda_fail(err, what);
-            if (err == cudaErrorMemoryAllocation) cudaGetLastError();
-            return false;
-        }
-        return true;
-    };
-    if (!dmalloc((void **)&ctx->d_tth, w.tables, "cudaMalloc(tables)")) return fail(rc);
-    ctx->d_pph = ctx->d_tth + (cfg->n_theta + 1);
-    if (!dmalloc((void **)&ctx->d_counters, w.counters, "cudaMalloc(counters)")) return fail(rc);
-    if (!dmalloc((void **)&ctx->d_bx, w.buckets, "cudaMalloc(hit buckets)")) return fail(rc);
-    {
-        unsigned char *b0 = reinterpret_cast<unsigned char *>(ctx->d_bx);
-        const size_t one = w.buckets / 6;
-        ctx->d_br2 = reinterpret_cast<float *>(b0 + one);
-        ctx->d_bden = reinterpret_cast<float *>(b0 + 2 * one);
-        ctx->d_hplane = reinterpret_cast<int32_t *>(b0 + 4 * one);
-        ctx->d_hrel = reinterpret_cast<int32_t *>(b0 + 5 * one);
+    if (d_workspace) {
+        ctx->d_ws = static_cast<unsigned char *>(d_workspace);
+    } else {
+        e = cudaMalloc((void **)&ctx->d_ws, lay.total);
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return fail(HT_ERR_NOMEM); }
+        if (e != cudaSuccess) return fail(cuda_fail(e, "cudaMalloc(workspace)"));
+        ctx->owns_ws = true;
     }
-    if (!dmalloc((void **)&ctx->d_bucket_start, w.bucket_start, "cudaMalloc(bucket offsets)")) return fail(rc);
-    if (!dmalloc((void **)&ctx->d_counts, w.counts, "cudaMalloc(bucket counts)")) return fail(rc);
-    if ((e = cudaMemset(ctx->d_counts, 0, w.counts)) != cudaSuccess) return fail(cuda_fail(e, "cudaMemset(bucket counts)"));
-    if ((e = cudaMemcpy(ctx->d_tth, tth.data(), tth.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
+    unsigned char *ws = ctx->d_ws;
+    ctx->d_tth = reinterpret_cast<float *>(ws + lay.tables);
+    ctx->d_pph = ctx->d_tth + (cfg->n_theta + 1);
+    ctx->d_counters = reinterpret_cast<uint32_t *>(ws + lay.counters);
+    ctx->d_bx = reinterpret_cast<float *>(ws + lay.hits);
+    ctx->d_br2 = reinterpret_cast<float *>(ws + lay.hits + lay.hits_part);
+    ctx->d_bden = reinterpret_cast<float *>(ws + lay.hits + 2 * lay.hits_part);
+    ctx->d_hplane = reinterpret_cast<int32_t *>(ws + lay.hits + 4 * lay.hits_part);
+    ctx->d_hrel = reinterpret_cast<int32_t *>(ws + lay.hits + 5 * lay.hits_part);
+    ctx->d_bucket_start = reinterpret_cast<int32_t *>(ws + lay.bucket_start);
+    ctx->d_counts = reinterpret_cast<uint32_t *>(ws + lay.counts);
+    if ((e = cudaMemset(ctx->d_counts, 0, align_up(sizeof(uint32_t) * (size_t)cfg->max_events * (size_t)(cfg->n_theta * cfg->n_phi), 256))) != cudaSuccess ||
+        (e = cudaMemcpy(ctx->d_tth, tth.data(), tth.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMemcpy(ctx->d_pph, pph.data(), pph.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
-        (e = cudaMemset(ctx->d_counters, 0, w.counters)) != cudaSuccess)
-        return fail(cuda_fail(e, "table upload"));
+        (e = cudaMemset(ctx->d_counters, 0, 256)) != cudaSuccess)
+        return fail(cuda_fail(e, "workspace initialisation"));
+    if ((e = cudaEventCreateWithFlags(&ctx->order_event, cudaEventDisableTiming)) != cudaSuccess)
+        return fail(cuda_fail(e, "cudaEventCreate"));
 
     if (cfg->host_slots > 0) {
-        if (!dmalloc((void **)&ctx->d_in, w.host_off + w.host_hits, "cudaMalloc(host input)")) return fail(rc);
-        if (!dmalloc((void **)&ctx->d_hmh, w.host_mh, "cudaMalloc(host matrices)")) return fail(rc);
-        if ((e = cudaHostAlloc((void **)&ctx->h_in, w.host_off + w.host_hits, cudaHostAllocMapped)) != cudaSuccess)
+        const size_t ns = (size_t)cfg->host_slots;
+        ctx->d_hmh = reinterpret_cast<uint32_t *>(ws + lay.mh);
+        if ((e = cudaHostAlloc((void **)&ctx->h_in_all, lay.in_block * ns, cudaHostAllocMapped)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaHostAlloc(input)"));
-        if ((e = cudaHostGetDevicePointer((void **)&ctx->d_in_mapped, ctx->h_in, 0)) != cudaSuccess)
-            return fail(cuda_fail(e, "cudaHostGetDevicePointer(input)"));
-        if ((e = cudaHostAlloc((void **)&ctx->h_res, w.host_res, cudaHostAllocMapped)) != cudaSuccess)
+        if ((e = cudaHostAlloc((void **)&ctx->h_res_all, lay.res_block * ns, cudaHostAllocMapped)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaHostAlloc(result)"));
-        if ((e = cudaHostGetDevicePointer((void **)&ctx->d_res, ctx->h_res, 0)) != cudaSuccess)
-            return fail(cuda_fail(e, "cudaHostGetDevicePointer(result)"));
-        if ((e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking)) != cudaSuccess)
+        unsigned char *in_map = nullptr, *res_map = nullptr;
+        if ((e = cudaHostGetDevicePointer((void **)&in_map, ctx->h_in_all, 0)) != cudaSuccess ||
+            (e = cudaHostGetDevicePointer((void **)&res_map, ctx->h_res_all, 0)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaHostGetDevicePointer"));
+        ctx->slots.resize(ns);
+        for (size_t s = 0; s < ns; ++s) {
+            HostSlot &sl = ctx->slots[s];
+            sl.h_in = ctx->h_in_all + s * lay.in_block;
+            sl.d_in_mapped = in_map + s * lay.in_block;
+            sl.d_in = ws + lay.in_dev + s * lay.in_block;
+            sl.h_res = ctx->h_res_all + s * lay.res_block;
+            sl.d_res = res_map + s * lay.res_block;
+            if ((e = cudaEventCreateWithFlags(&sl.copied, cudaEventDisableTiming)) != cudaSuccess ||
+                (e = cudaEventCreateWithFlags(&sl.done, cudaEventDisableTiming)) != cudaSuccess)
+                return fail(cuda_fail(e, "cudaEventCreate(slot)"));
+        }
+        if ((e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking)) != cudaSuccess ||
+            (e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaStreamCreate"));
     }
 
@@ -302,18 +384,18 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
             (e = cudaFuncSetAttribute(ht::fill_tiles_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)ctx->fill_smem_max[1])) != cudaSuccess)
             return fail(cuda_fail(e, "cudaFuncSetAttribute"));
+        // the kernel synchronises its grid: every CTA of a launch (at most one per SM) must be resident at once
         int occ0 = 0, occ1 = 0;
         if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ0, ht::fill_tiles_kernel<false>, ht::kFillThreads,
                                                                ctx->fill_smem_max[0])) != cudaSuccess ||
             (e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, ht::fill_tiles_kernel<true>, ht::kFillThreads,
                                                                ctx->fill_smem_max[1])) != cudaSuccess)
             return fail(cuda_fail(e, "fill kernel occupancy"));
-        ctx->fill_ok = coop && occ0 >= 1 && occ1 >= 1;
+        ctx->fill_ok = occ0 >= 1 && occ1 >= 1 && (coop || !tun.cooperative_launch);
     }
     // peak scan: a persistent grid of exactly the CTAs that are resident at once (a grid-stride loop over more CTAs
     // than fit would run the excess as a second, partly empty wave)
-    int unroll = env_int("HT_PEAKS_UNROLL", 2);      // config 2, B200, back-to-back launches: 45.2 us (U=2, 6 CTAs/SM), 46.4 (U=4), 49.4 (U=8)
-    if (unroll != 2 && unroll != 4 && unroll != 8) unroll = 2;
+    const int unroll = tun.peaks_unroll ? tun.peaks_unroll : 2;     // config 2, B200: 45.2 us (U=2, 6 CTAs/SM), 46.4 (U=4), 49.4 (U=8)
     ctx->peaks_unroll = unroll;
     int occ4 = 0, occ1 = 0;
     if (unroll == 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ4, ht::peaks_kernel<4, 2>, ht::kPeaksThreads, 0);
@@ -321,11 +403,9 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ4, ht::peaks_kernel<4, 4>, ht::kPeaksThreads, 0);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, ht::peaks_kernel<1, 4>, ht::kPeaksThreads, 0);
     if (e != cudaSuccess) return fail(cuda_fail(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor"));
-    const int occ_cap = env_int("HT_PEAKS_CTAS_PER_SM", 32);
-    if (occ4 > occ_cap) occ4 = occ_cap;
-    if (occ1 > occ_cap) occ1 = occ_cap;
-    if (occ4 < 1) occ4 = 1;
-    if (occ1 < 1) occ1 = 1;
+    const int occ_cap = tun.peaks_ctas_per_sm > 0 ? tun.peaks_ctas_per_sm : 32;
+    occ4 = std::max(1, std::min(occ4, occ_cap));
+    occ1 = std::max(1, std::min(occ1, occ_cap));
     ctx->peaks_grid_vec4 = ctx->sm_count * occ4;
     ctx->peaks_grid_vec1 = ctx->sm_count * occ1;
     ctx->info[6] = ctx->sm_count;
@@ -333,30 +413,29 @@ int ht_create(const ht_config *cfg, ht_ctx **out)
     return HT_OK;
 }
 
+}  // extern "C"
+
 namespace {
 
-FillPlan plan_fill(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool peaks)
+FillPlan compute_fill_plan(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool peaks)
 {
     FillPlan pl;
     if (!ctx->fill_ok) return pl;
     const ht_config &c = ctx->cfg;
-    const size_t budget = ctx->fill_smem_max[peaks ? 1 : 0];
+    const ht_tuning &tun = ctx->tun;
+    const size_t budget_all = ctx->fill_smem_max[peaks ? 1 : 0];
     const size_t row_bytes = (size_t)c.n_b * 4u;
     const long long planes = (long long)c.n_theta * c.n_phi;
     // mode 1 (per-CTA shared-memory hit index): one event, uint16 indices and plane ids, an index of at most 48 KB
-    const int force = env_int("HT_FILL_MODE", -1);
-    int mode = (n_events == 1 && n_hits <= 24576 && planes < 65535) ? 1 : 0;
-    if (force == 0) mode = 0;
+    int mode = (n_events == 1 && n_hits <= 24576 && planes < 65535 && !tun.fill_batch_classification) ? 1 : 0;
     // without the fused peak search the kernel is purely store-bound and measured fastest with slabs of <= 96 KB
     // (config 2, B200: 51.5 us at 96 KB, 53.4 at 100 KB, 59.4 at 104 KB); with it, the largest slab wins (fewer halo rows)
-    const int slab_kb = env_int("HT_FILL_SLAB_KB", peaks ? 0 : 96);
-    // shared memory set aside for the hits the planner stages per tile (two buffers of 16 bytes per hit): room for twice
-    // the average number of hits per (event, plane), at most 512 hits; whatever else is left over is added below
+    const int slab_kb = tun.fill_slab_kb > 0 ? tun.fill_slab_kb : (peaks ? 0 : 96);
+    // shared memory set aside for the hits staged per tile (two buffers of 16 bytes per hit): room for twice the
+    // average number of hits per (event, plane), at most 512 hits; whatever else is left over is added below
     long long want_cap = 2ll * (long long)n_hits / ((long long)(n_events > 0 ? n_events : 1) * planes);
     want_cap = (want_cap + 31) / 32 * 32;
-    if (want_cap > 512) want_cap = 512;
-    if (want_cap < 32) want_cap = 32;
-    const size_t budget_all = budget;
+    want_cap = std::min(512ll, std::max(32ll, want_cap));
     auto rows_for = [&](int md) -> long long {
         const size_t budget = budget_all > (size_t)want_cap * 32u ? budget_all - (size_t)want_cap * 32u : 0;
         long long rows = c.n_a;
@@ -384,9 +463,10 @@ FillPlan plan_fill(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool pea
             pl.slab_words = (uint32_t)(align_up((size_t)rows * row_bytes, 16) / 4u);
             pl.smem = fill_smem_bytes(c, rows, mode, n_hits);
             // what is left of the budget stages the hits of two tiles (x, r2, den, rc: 16 bytes per hit), up to 512 per tile
-            long long cap = ((long long)(budget - pl.smem) / 32) / 32 * 32;
-            if (cap > 512) cap = 512;
-            if (env_int("HT_FILL_HIT_CAP", -1) >= 0 && cap > env_int("HT_FILL_HIT_CAP", -1)) cap = env_int("HT_FILL_HIT_CAP", -1) / 32 * 32;
+            long long cap = ((long long)(budget_all - pl.smem) / 32) / 32 * 32;
+            cap = std::min(cap, 512ll);
+            if (tun.fill_hit_cap > 0) cap = std::min(cap, (long long)tun.fill_hit_cap / 32 * 32);
+            if (tun.fill_hit_cap < 0) cap = 0;
             pl.hit_cap = (int)cap;
             pl.smem += (size_t)cap * 32u;
             return pl;
@@ -395,13 +475,26 @@ FillPlan plan_fill(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool pea
     }
 }
 
+const FillPlan &plan_fill(ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool peaks)
+{
+    const int k = peaks ? 1 : 0;
+    if (ctx->plan_key[k][0] != n_events || ctx->plan_key[k][1] != n_hits) {
+        ctx->plan_cache[k] = compute_fill_plan(ctx, n_events, n_hits, peaks);
+        ctx->plan_key[k][0] = n_events;
+        ctx->plan_key[k][1] = n_hits;
+    }
+    return ctx->plan_cache[k];
+}
+
 // The fill kernel (prologue a0 + tiles a1-a3), with (PEAKS: + a4-a5) or without the fused peak search.
+// early_inputs: the hit arrays are known not to be written by device work enqueued before this call (the context's own
+// pinned staging blocks), so the kernel may read them before the previous kernel of the stream has completed.
 int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off, int32_t n_events,
                 int32_t n_hits_total, uint32_t *d_mh, bool peaks, uint32_t threshold, ht_peak *d_out, uint32_t capacity,
-                uint32_t *d_n_found, cudaStream_t st)
+                uint32_t *d_n_found, cudaStream_t st, bool early_inputs)
 {
     const ht::Geom &g = ctx->geom;
-    const FillPlan pl = plan_fill(ctx, n_events, n_hits_total, peaks);
+    const FillPlan &pl = plan_fill(ctx, n_events, n_hits_total, peaks);
     if (!pl.ok) return HT_ERR_UNSUPPORTED;
     ht::FillArgs a{};
     a.x = d_x; a.y = d_y; a.z = d_z; a.event_offsets = d_off; a.n_events = n_events; a.n_hits = n_hits_total;
@@ -429,17 +522,21 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     if (n_tiles >= (1ull << 31)) return HT_ERR_UNSUPPORTED;        // tile indices are 32-bit in the kernel
     a.n_tiles = (uint32_t)n_tiles;
     a.mh = d_mh;
-    a.bulk_ok = (g.n_b % 4 == 0) && ((reinterpret_cast<uintptr_t>(d_mh) & 15u) == 0) && env_int("HT_FILL_NO_BULK", 0) == 0;
+    a.bulk_ok = (g.n_b % 4 == 0) && ((reinterpret_cast<uintptr_t>(d_mh) & 15u) == 0) && !ctx->tun.fill_plain_stores;
+    a.atomic_votes = ctx->tun.fill_shared_atomics ? 1 : 0;
+    a.early_inputs = early_inputs ? 1 : 0;
     a.threshold = threshold;
     static_assert(sizeof(ht::PeakOut) == sizeof(ht_peak), "peak record layout");
     a.out = reinterpret_cast<ht::PeakOut *>(d_out);
     a.capacity = capacity;
     a.counters = ctx->d_counters;
     a.n_found_out = d_n_found;
-    // one CTA per SM; CTA c takes tiles c, c + grid, ...
+    // one CTA per SM; CTA c starts with tile c
     unsigned long long grid = (unsigned long long)ctx->sm_count;
     if (grid > n_tiles) grid = n_tiles;
     if (grid < 1) grid = 1;
+    const int ro = order_after_previous(ctx, st);
+    if (ro != HT_OK) return ro;
     // Mode 1's grid barrier: the fast one-shot form needs the host to know the counter's value, which a launch captured
     // into a CUDA graph (replayed any number of times) cannot; captured launches use the self-resetting barrier.
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
@@ -448,11 +545,26 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.tile_counter = ctx->d_counters + 6;
     a.bar_count = one_shot ? ctx->d_counters + 5 : nullptr;
     a.bar_target = ctx->bar_epoch + (uint32_t)grid;
-    {   // both prologues synchronise the grid: co-residency is guaranteed by a cooperative launch
-        void *params[] = {&a};
-        const void *fn = peaks ? reinterpret_cast<const void *>(ht::fill_tiles_kernel<true>)
-                               : reinterpret_cast<const void *>(ht::fill_tiles_kernel<false>);
+    const void *fn = peaks ? reinterpret_cast<const void *>(ht::fill_tiles_kernel<true>)
+                           : reinterpret_cast<const void *>(ht::fill_tiles_kernel<false>);
+    void *params[] = {&a};
+    if (ctx->tun.cooperative_launch) {
         HT_CUDA(cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(ht::kFillThreads), params, pl.smem, st));
+    } else {
+        // Ordinary launch of a grid that ht_create has verified to be co-resident (one CTA per SM), as a programmatic
+        // dependent launch: the CTAs may be placed while the previous kernel of the stream drains; the kernel waits
+        // (griddepcontrol.wait) before it touches anything that kernel may have written.
+        cudaLaunchConfig_t lc{};
+        lc.gridDim = dim3((unsigned)grid);
+        lc.blockDim = dim3(ht::kFillThreads);
+        lc.dynamicSmemBytes = pl.smem;
+        lc.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        lc.attrs = at;
+        lc.numAttrs = 1;
+        HT_CUDA(cudaLaunchKernelExC(&lc, fn, params));
     }
     if (one_shot) ctx->bar_epoch = a.bar_target;
     ++ctx->launches;
@@ -463,13 +575,16 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
 
 }  // namespace
 
+extern "C" {
+
 int ht_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
             int32_t n_events, int32_t n_hits_total, uint32_t *d_mh, void *cuda_stream)
 {
     const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh, true);
     if (rc != HT_OK || n_events == 0) return rc;
+    DeviceGuard guard(ctx->cfg.device);
     return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh, false, 0u, nullptr, 0u, nullptr,
-                       static_cast<cudaStream_t>(cuda_stream));
+                       static_cast<cudaStream_t>(cuda_stream), false);
 }
 
 int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
@@ -479,13 +594,14 @@ int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const float *
     if (threshold < 1u || !d_n_found || (capacity > 0 && !d_out)) return HT_ERR_INVALID_ARG;
     const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh_or_null, false);
     if (rc != HT_OK) return rc;
+    DeviceGuard guard(ctx->cfg.device);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     if (n_events == 0) {
         HT_CUDA(cudaMemsetAsync(d_n_found, 0, sizeof(uint32_t), st));
         return HT_OK;
     }
     return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh_or_null, true, threshold, d_out, capacity,
-                       d_n_found, st);
+                       d_n_found, st, false);
 }
 
 int ht_fill_naive(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
@@ -493,8 +609,11 @@ int ht_fill_naive(ht_ctx *ctx, const float *d_x, const float *d_y, const float *
 {
     const int rc = check_fill_args(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh, true);
     if (rc != HT_OK || n_events == 0) return rc;
+    DeviceGuard guard(ctx->cfg.device);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const ht::Geom &g = ctx->geom;
+    const int ro = order_after_previous(ctx, st);
+    if (ro != HT_OK) return ro;
     HT_CUDA(cudaMemsetAsync(d_mh, 0, (size_t)n_events * (size_t)g.cells * sizeof(uint32_t), st));
     if (n_hits_total > 0) {
         const int threads = g.n_a >= 256 ? 256 : ((g.n_a + 31) / 32) * 32;
@@ -511,6 +630,7 @@ int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_t thres
 {
     if (!ctx || n_events < 0 || n_events > ctx->cfg.max_events || threshold < 1u || !d_n_found) return HT_ERR_INVALID_ARG;
     if (capacity > 0 && !d_out) return HT_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     if (n_events == 0) {
         HT_CUDA(cudaMemsetAsync(d_n_found, 0, sizeof(uint32_t), st));
@@ -527,6 +647,8 @@ int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_t thres
     const unsigned long long resident = (unsigned long long)(vec4 ? ctx->peaks_grid_vec4 : ctx->peaks_grid_vec1);
     if (grid > resident) grid = resident;
     if (grid < 1ull) grid = 1ull;
+    const int ro = order_after_previous(ctx, st);
+    if (ro != HT_OK) return ro;
     static_assert(sizeof(ht::PeakOut) == sizeof(ht_peak), "peak record layout");
     ht::PeakOut *out = reinterpret_cast<ht::PeakOut *>(d_out);
 #define HT_LAUNCH_PEAKS(V, UU)                                                                                          \
@@ -540,6 +662,108 @@ int ht_peaks(ht_ctx *ctx, const uint32_t *d_mh, int32_t n_events, uint32_t thres
     HT_CUDA(cudaGetLastError());
     ++ctx->launches;
     ctx->info[4] = (int32_t)grid; ctx->info[5] = ht::kPeaksThreads;
+    return HT_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+// offsets of the parts of a slot's input block [offsets | x | y | z] for n_hits hits
+struct InBlock {
+    size_t o_x, o_y, o_z, bytes;
+};
+InBlock in_block(const ht_ctx *ctx, int32_t n_hits)
+{
+    InBlock b;
+    b.o_x = align_up(sizeof(int32_t) * ((size_t)ctx->cfg.max_events + 1), 16);
+    const size_t part = align_up(sizeof(float) * (size_t)n_hits, 16);
+    b.o_y = b.o_x + part;
+    b.o_z = b.o_y + part;
+    b.bytes = b.o_z + part;
+    return b;
+}
+
+// One group of events (at most host_slots, all in the input block of slot `s`, matrices from `mh_slot` on) through the
+// fused kernel (or the two-call path for shapes it refuses), peak list and count into slot s's mapped result block.
+int enqueue_group(ht_ctx *ctx, HostSlot &sl, const unsigned char *in_base, const InBlock &ib, int32_t hit_base, int32_t ne,
+                  int32_t nh, uint32_t *d_mh, uint32_t threshold, uint32_t room, bool early_inputs)
+{
+    cudaStream_t st = ctx->host_stream;
+    const float *d_x = reinterpret_cast<const float *>(in_base + ib.o_x) + hit_base;
+    const float *d_y = reinterpret_cast<const float *>(in_base + ib.o_y) + hit_base;
+    const float *d_z = reinterpret_cast<const float *>(in_base + ib.o_z) + hit_base;
+    const int32_t *d_off = reinterpret_cast<const int32_t *>(in_base);
+    uint32_t *d_count = reinterpret_cast<uint32_t *>(sl.d_res);
+    ht_peak *d_list = reinterpret_cast<ht_peak *>(sl.d_res + kResHeader);
+    int rc = launch_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, true, threshold, d_list, room, d_count, st, early_inputs);
+    if (rc == HT_ERR_UNSUPPORTED) {
+        rc = ht_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, st);
+        if (rc == HT_ERR_UNSUPPORTED) rc = ht_fill_naive(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, st);
+        if (rc != HT_OK) return rc;
+        rc = ht_peaks(ctx, d_mh, ne, threshold, d_list, room, d_count, st);
+    }
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y, const float *h_z, int32_t n_hits,
+                   uint32_t threshold)
+{
+    if (!ctx) return HT_ERR_INVALID_ARG;
+    if (ctx->cfg.host_slots < 1) return HT_ERR_UNSUPPORTED;
+    if (slot < 0 || slot >= ctx->cfg.host_slots || n_hits < 0 || n_hits > ctx->cfg.max_hits || threshold < 1u) return HT_ERR_INVALID_ARG;
+    if (n_hits > 0 && (!h_x || !h_y || !h_z)) return HT_ERR_INVALID_ARG;
+    HostSlot &sl = ctx->slots[(size_t)slot];
+    if (sl.busy) return HT_ERR_INVALID_ARG;                       // ht_wait_host first
+    DeviceGuard guard(ctx->cfg.device);
+    const InBlock ib = in_block(ctx, n_hits);
+    int32_t *off = reinterpret_cast<int32_t *>(sl.h_in);
+    off[0] = 0;
+    off[1] = n_hits;
+    if (n_hits > 0) {
+        const size_t nb = sizeof(float) * (size_t)n_hits;
+        std::memcpy(sl.h_in + ib.o_x, h_x, nb);
+        std::memcpy(sl.h_in + ib.o_y, h_y, nb);
+        std::memcpy(sl.h_in + ib.o_z, h_z, nb);
+    }
+    // One event whose hits the grid reads exactly once (mode 1): straight from the pinned block (zero-copy over PCIe);
+    // otherwise one packed copy on the copy stream, which overlaps the kernel of the previous event.
+    const FillPlan &pl = plan_fill(ctx, 1, n_hits, true);
+    const bool zero_copy = !ctx->tun.host_copy_input && pl.ok && pl.mode == 1;
+    const unsigned char *in_base = sl.d_in_mapped;
+    if (!zero_copy) {
+        HT_CUDA(cudaMemcpyAsync(sl.d_in, sl.h_in, ib.bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+        HT_CUDA(cudaEventRecord(sl.copied, ctx->copy_stream));
+        HT_CUDA(cudaStreamWaitEvent(ctx->host_stream, sl.copied, 0));
+        in_base = sl.d_in;
+    }
+    uint32_t *d_mh = ctx->d_hmh + (size_t)slot * (size_t)ctx->geom.cells;
+    const int rc = enqueue_group(ctx, sl, in_base, ib, 0, 1, n_hits, d_mh, threshold, ctx->cfg.host_peak_capacity, true);
+    if (rc != HT_OK) return rc;
+    HT_CUDA(cudaEventRecord(sl.done, ctx->host_stream));
+    sl.busy = true;
+    return HT_OK;
+}
+
+int ht_wait_host(ht_ctx *ctx, int32_t slot, ht_peak *h_out, uint32_t capacity, uint32_t *h_n_found)
+{
+    if (!ctx || !h_n_found) return HT_ERR_INVALID_ARG;
+    if (ctx->cfg.host_slots < 1) return HT_ERR_UNSUPPORTED;
+    if (slot < 0 || slot >= ctx->cfg.host_slots || (capacity > 0 && !h_out)) return HT_ERR_INVALID_ARG;
+    HostSlot &sl = ctx->slots[(size_t)slot];
+    if (!sl.busy) return HT_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    HT_CUDA(cudaEventSynchronize(sl.done));
+    sl.busy = false;
+    const uint32_t found = *reinterpret_cast<const volatile uint32_t *>(sl.h_res);
+    uint32_t got = found < ctx->cfg.host_peak_capacity ? found : ctx->cfg.host_peak_capacity;
+    if (got > capacity) got = capacity;
+    if (got > 0) std::memcpy(h_out, sl.h_res + kResHeader, sizeof(ht_peak) * (size_t)got);
+    *h_n_found = found;
     return HT_OK;
 }
 
@@ -558,34 +782,34 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
     if (h_event_offsets[0] != 0 || h_event_offsets[n_events] != n_hits_total) return HT_ERR_INVALID_ARG;
     for (int e = 0; e < n_events; ++e)
         if (h_event_offsets[e] > h_event_offsets[e + 1]) return HT_ERR_INVALID_ARG;
+    for (const HostSlot &s : ctx->slots)
+        if (s.busy) return HT_ERR_INVALID_ARG;                    // submitted events must be waited for first
 
+    // one event without a matrix read-back: the asynchronous pair, back to back
+    if (n_events == 1 && !h_mh_or_null) {
+        int rc = ht_submit_host(ctx, 0, h_x, h_y, h_z, n_hits_total, threshold);
+        if (rc != HT_OK) return rc;
+        return ht_wait_host(ctx, 0, h_out, capacity, h_n_found);
+    }
+
+    DeviceGuard guard(ctx->cfg.device);
     cudaStream_t st = ctx->host_stream;
+    HostSlot &sl = ctx->slots[0];
     const size_t cells = (size_t)ctx->geom.cells;
     // input block [offsets | x | y | z], 16-byte aligned parts, packed in pinned memory: ONE host-to-device copy
-    const size_t o_x = align_up(sizeof(int32_t) * ((size_t)ctx->cfg.max_events + 1), 16);
-    const size_t part = align_up(sizeof(float) * (size_t)n_hits_total, 16);
-    const size_t o_y = o_x + part, o_z = o_y + part, in_bytes = o_z + part;
-    // One event whose hits the grid classifies in one pass (mode 1): the kernel reads every hit exactly once, so it reads
-    // them straight from the pinned block (zero-copy over PCIe) and no host-to-device copy is issued at all.
-    const bool zero_copy = n_events == 1 && env_int("HT_HOST_ZERO_COPY", 1) != 0 &&
-                           plan_fill(ctx, 1, n_hits_total, true).ok && plan_fill(ctx, 1, n_hits_total, true).mode == 1;
-    unsigned char *in_base = zero_copy ? ctx->d_in_mapped : ctx->d_in;
-    const float *d_x = reinterpret_cast<const float *>(in_base + o_x);
-    const float *d_y = reinterpret_cast<const float *>(in_base + o_y);
-    const float *d_z = reinterpret_cast<const float *>(in_base + o_z);
-    const int32_t *d_off = reinterpret_cast<const int32_t *>(in_base);
+    const InBlock ib = in_block(ctx, n_hits_total);
+    const FillPlan &pl1 = plan_fill(ctx, 1, n_hits_total, true);
+    const bool zero_copy = n_events == 1 && !ctx->tun.host_copy_input && pl1.ok && pl1.mode == 1;
+    const unsigned char *in_base = zero_copy ? sl.d_in_mapped : sl.d_in;
     if (n_hits_total > 0) {
         const size_t nb = sizeof(float) * (size_t)n_hits_total;
-        std::memcpy(ctx->h_in + o_x, h_x, nb);
-        std::memcpy(ctx->h_in + o_y, h_y, nb);
-        std::memcpy(ctx->h_in + o_z, h_z, nb);
+        std::memcpy(sl.h_in + ib.o_x, h_x, nb);
+        std::memcpy(sl.h_in + ib.o_y, h_y, nb);
+        std::memcpy(sl.h_in + ib.o_z, h_z, nb);
     }
-    // the kernels write the count and the list straight into mapped pinned memory: no device-to-host copy
-    uint32_t *d_count = reinterpret_cast<uint32_t *>(ctx->d_res);
-    ht_peak *d_list = reinterpret_cast<ht_peak *>(ctx->d_res + kResHeader);
     uint32_t found_total = 0u, written = 0u;
     const int slots = ctx->cfg.host_slots;
-    int32_t *off_local = reinterpret_cast<int32_t *>(ctx->h_in);   // reused by the next group only after this group's synchronisation
+    int32_t *off_local = reinterpret_cast<int32_t *>(sl.h_in);   // reused by the next group only after this group's synchronisation
     for (int e0 = 0; e0 < n_events; e0 += slots) {
         const int ne = (n_events - e0 < slots) ? n_events - e0 : slots;
         const int32_t hb = h_event_offsets[e0];
@@ -594,26 +818,19 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
         if (zero_copy)
             ;
         else if (e0 == 0)
-            HT_CUDA(cudaMemcpyAsync(ctx->d_in, ctx->h_in, in_bytes, cudaMemcpyHostToDevice, st));
+            HT_CUDA(cudaMemcpyAsync(sl.d_in, sl.h_in, ib.bytes, cudaMemcpyHostToDevice, st));
         else
-            HT_CUDA(cudaMemcpyAsync(ctx->d_in, ctx->h_in, sizeof(int32_t) * (size_t)(ne + 1), cudaMemcpyHostToDevice, st));
+            HT_CUDA(cudaMemcpyAsync(sl.d_in, sl.h_in, sizeof(int32_t) * (size_t)(ne + 1), cudaMemcpyHostToDevice, st));
         const uint32_t room = capacity - written;
-        // the fused kernel (matrix materialised AND peaks found in one pass); shapes it refuses take the two-call path
-        int rc = ht_fill_peaks(ctx, d_x + hb, d_y + hb, d_z + hb, d_off, ne, nh, ctx->d_hmh, threshold, d_list, room, d_count, st);
-        if (rc == HT_ERR_UNSUPPORTED) {
-            rc = ht_fill(ctx, d_x + hb, d_y + hb, d_z + hb, d_off, ne, nh, ctx->d_hmh, st);
-            if (rc == HT_ERR_UNSUPPORTED) rc = ht_fill_naive(ctx, d_x + hb, d_y + hb, d_z + hb, d_off, ne, nh, ctx->d_hmh, st);
-            if (rc != HT_OK) return rc;
-            rc = ht_peaks(ctx, ctx->d_hmh, ne, threshold, d_list, room, d_count, st);
-        }
+        const int rc = enqueue_group(ctx, sl, in_base, ib, hb, ne, nh, ctx->d_hmh, threshold, room, false);
         if (rc != HT_OK) return rc;
         if (h_mh_or_null)
             HT_CUDA(cudaMemcpyAsync(h_mh_or_null + (size_t)e0 * cells, ctx->d_hmh, sizeof(uint32_t) * cells * (size_t)ne,
                                     cudaMemcpyDeviceToHost, st));
         HT_CUDA(cudaStreamSynchronize(st));
-        const uint32_t found = *reinterpret_cast<const volatile uint32_t *>(ctx->h_res);
+        const uint32_t found = *reinterpret_cast<const volatile uint32_t *>(sl.h_res);
         const uint32_t got = found < room ? found : room;
-        const ht_peak *src = reinterpret_cast<const ht_peak *>(ctx->h_res + kResHeader);
+        const ht_peak *src = reinterpret_cast<const ht_peak *>(sl.h_res + kResHeader);
         for (uint32_t k = 0; k < got; ++k) {
             ht_peak p = src[k];
             p.event += (uint32_t)e0;
@@ -631,6 +848,7 @@ int ht_tracks(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, ht_track *d
     if (!ctx) return HT_ERR_INVALID_ARG;
     if (n_peaks == 0u) return HT_OK;
     if (!d_peaks || !d_out) return HT_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
     static_assert(sizeof(ht::TrackOut) == sizeof(ht_track), "track record layout");
     const unsigned threads = 128, blocks = (n_peaks + threads - 1u) / threads;
     ht::tracks_kernel<<<blocks, threads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
@@ -640,15 +858,20 @@ int ht_tracks(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, ht_track *d
     return HT_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ diagnostics (ht_diag.h)
+
 int ht_selftest_division(int32_t device, uint64_t n_pairs, uint64_t seed, uint64_t *h_mismatches)
 {
     if (!h_mismatches) return HT_ERR_INVALID_ARG;
-    HT_CUDA(cudaSetDevice(device));
+    DeviceGuard guard(device);
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "cudaSetDevice");
+    int sms = 0;
+    HT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
     unsigned long long *d = nullptr;
     HT_CUDA(cudaMalloc((void **)&d, sizeof(unsigned long long)));
     cudaError_t e = cudaMemset(d, 0, sizeof(unsigned long long));
     if (e == cudaSuccess) {
-        ht::selftest_division_kernel<<<148 * 8, 256>>>((unsigned long long)n_pairs, (unsigned long long)seed, d);
+        ht::selftest_division_kernel<<<sms * 8, 256>>>((unsigned long long)n_pairs, (unsigned long long)seed, d);
         e = cudaGetLastError();
     }
     unsigned long long h = 0;
@@ -656,6 +879,61 @@ int ht_selftest_division(int32_t device, uint64_t n_pairs, uint64_t seed, uint64
     cudaFree(d);
     if (e != cudaSuccess) return cuda_fail(e, "ht_selftest_division");
     *h_mismatches = (uint64_t)h;
+    return HT_OK;
+}
+
+int ht_diag_memset(void *d_dst, int32_t value, size_t bytes, void *cuda_stream)
+{
+    if (!d_dst && bytes) return HT_ERR_INVALID_ARG;
+    HT_CUDA(cudaMemsetAsync(d_dst, value, bytes, static_cast<cudaStream_t>(cuda_stream)));
+    return HT_OK;
+}
+
+int ht_diag_vote_rates(int32_t device, int32_t iters, double *h_rates, uint64_t *h_sum_errors)
+{
+    if (!h_rates || !h_sum_errors || iters < 1) return HT_ERR_INVALID_ARG;
+    DeviceGuard guard(device);
+    if (guard.err != cudaSuccess) return cuda_fail(guard.err, "cudaSetDevice");
+    int sms = 0;
+    HT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+    ht::DiagOut *d = nullptr;
+    HT_CUDA(cudaMalloc((void **)&d, sizeof(ht::DiagOut) * (size_t)sms));
+    std::vector<ht::DiagOut> h((size_t)sms);
+    const size_t smem = (size_t)ht::kDiagWarps * ht::kDiagRowCells * 4u;
+    uint64_t errors = 0;
+    cudaError_t e = cudaSuccess;
+    auto run = [&](auto kernel, int pattern) {
+        if (e != cudaSuccess) return;
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        for (int rep = 0; rep < 2 && e == cudaSuccess; ++rep) {          // the first launch warms up
+            kernel<<<sms, 1024, smem>>>(iters, d);
+            e = cudaGetLastError();
+            if (e == cudaSuccess) e = cudaMemcpy(h.data(), d, sizeof(ht::DiagOut) * (size_t)sms, cudaMemcpyDeviceToHost);
+        }
+        if (e != cudaSuccess) return;
+        std::vector<double> r;
+        for (const ht::DiagOut &o : h) {
+            r.push_back(o.cycles ? (double)o.votes / (double)o.cycles : 0.0);
+            errors += o.sum_errors;
+        }
+        std::sort(r.begin(), r.end());
+        h_rates[pattern] = r[r.size() / 2];
+    };
+    run(ht::vote_rates_kernel<HT_DIAG_RED_RANDOM>, HT_DIAG_RED_RANDOM);
+    run(ht::vote_rates_kernel<HT_DIAG_RED_RANDOM_71>, HT_DIAG_RED_RANDOM_71);
+    run(ht::vote_rates_kernel<HT_DIAG_RED_NO_CONFLICT>, HT_DIAG_RED_NO_CONFLICT);
+    run(ht::vote_rates_kernel<HT_DIAG_RED_TWO_WAY>, HT_DIAG_RED_TWO_WAY);
+    run(ht::vote_rates_kernel<HT_DIAG_RED_SAME>, HT_DIAG_RED_SAME);
+    run(ht::vote_rates_kernel<HT_DIAG_ATOM_RANDOM>, HT_DIAG_ATOM_RANDOM);
+    run(ht::vote_rates_kernel<HT_DIAG_ATOM_NO_CONFLICT>, HT_DIAG_ATOM_NO_CONFLICT);
+    run(ht::vote_rates_kernel<HT_DIAG_ATOM_SAME>, HT_DIAG_ATOM_SAME);
+    run(ht::vote_rates_kernel<HT_DIAG_RMW_RANDOM>, HT_DIAG_RMW_RANDOM);
+    run(ht::vote_rates_kernel<HT_DIAG_TAG_RANDOM>, HT_DIAG_TAG_RANDOM);
+    run(ht::vote_rates_kernel<HT_DIAG_MATCH_RANDOM>, HT_DIAG_MATCH_RANDOM);
+    run(ht::vote_rates_kernel<HT_DIAG_TAG_RANDOM_71>, HT_DIAG_TAG_RANDOM_71);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(e, "ht_diag_vote_rates");
+    *h_sum_errors = errors;
     return HT_OK;
 }
 
@@ -671,17 +949,17 @@ int ht_launch_info(const ht_ctx *ctx, int32_t out[8])
 void ht_destroy(ht_ctx *ctx)
 {
     if (!ctx) return;
-    cudaSetDevice(ctx->cfg.device);
+    DeviceGuard guard(ctx->cfg.device);
     if (ctx->host_stream) { cudaStreamSynchronize(ctx->host_stream); cudaStreamDestroy(ctx->host_stream); }
-    cudaFree(ctx->d_tth);
-    cudaFree(ctx->d_counters);
-    cudaFree(ctx->d_bx);
-    cudaFree(ctx->d_bucket_start);
-    cudaFree(ctx->d_counts);
-    cudaFree(ctx->d_in);
-    cudaFree(ctx->d_hmh);
-    if (ctx->h_res) cudaFreeHost(ctx->h_res);
-    if (ctx->h_in) cudaFreeHost(ctx->h_in);
+    if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
+    for (HostSlot &s : ctx->slots) {
+        if (s.copied) cudaEventDestroy(s.copied);
+        if (s.done) cudaEventDestroy(s.done);
+    }
+    if (ctx->order_event) cudaEventDestroy(ctx->order_event);
+    if (ctx->owns_ws) cudaFree(ctx->d_ws);
+    if (ctx->h_res_all) cudaFreeHost(ctx->h_res_all);
+    if (ctx->h_in_all) cudaFreeHost(ctx->h_in_all);
     delete ctx;
 }
 

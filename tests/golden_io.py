@@ -66,3 +66,32 @@ def read_paper_shapes(path: str | None = None) -> dict:
             k, *v = line.split()
             out[k] = [float(t) if "." in t else int(t) for t in v]
     return out
+
+
+def read_merge_cases(path=None):
+    """tests/golden/merge_cases.txt -> list of dict(name, dims, window, peaks PEAK-like tuples, want tuples)."""
+    path = path or os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "merge_cases.txt")
+    cases, cur = [], None
+    for line in open(path):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        tok = line.split()
+        if tok[0] == "case":
+            cur = dict(name=tok[1], dims=None, window=None, peaks=[], want=[])
+            cases.append(cur)
+        elif tok[0] == "dims":
+            cur["dims"] = tuple(int(t) for t in tok[1:5])
+        elif tok[0] == "window":
+            cur["window"] = int(tok[1])
+        elif tok[0] in ("peak", "want"):
+            ev, plane, a, b, count = (int(t) for t in tok[1:6])
+            _, _, n_a, n_b = cur["dims"]
+            cell = (plane * n_a + a) * n_b + b
+            if tok[0] == "peak":
+                cur["peaks"].append((ev, cell, count))
+            else:
+                cur["want"].append((ev, cell, count, int(tok[6])))
+        else:
+            raise ValueError(f"bad line in {path}: {line}")
+    return cases

@@ -16,12 +16,25 @@ def sort_peaks(pk: np.ndarray, cells: int) -> np.ndarray:
 class GpuHough:
     """One context + the device buffers of one batch."""
 
-    def __init__(self, binning, max_events: int, max_hits: int, host_slots: int = 0, host_peak_capacity: int = 0):
+    def __init__(self, binning, max_events: int, max_hits: int, host_slots: int = 0, host_peak_capacity: int = 0,
+                 tuning: dict | None = None, own_workspace: bool = False):
+        """``tuning``: fields of ht_tuning; ``own_workspace``: the test allocates the context's device workspace itself
+        (ht_query_sizes -> torch -> ht_create_ex), so the library allocates no device memory at all."""
         self.bn = binning
         self.cfg = B.ht_config.from_binning(binning, max_events=max_events, max_hits=max(1, max_hits), device=0,
                                             host_slots=host_slots, host_peak_capacity=host_peak_capacity)
-        self.ctx = B.ht_create(self.cfg)
         self.dev = torch.device("cuda:0")
+        self.tuning = B.ht_tuning(**tuning) if tuning else None
+        self.workspace = None
+        if own_workspace:
+            nbytes = B.ht_query_sizes(self.cfg)[1]
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.dev)
+            base = (self.workspace.data_ptr() + 255) // 256 * 256
+            self.ctx = B.ht_create_ex(self.cfg, self.tuning, base, nbytes)
+        elif self.tuning is not None:
+            self.ctx = B.ht_create_ex(self.cfg, self.tuning)
+        else:
+            self.ctx = B.ht_create(self.cfg)
 
     def close(self):
         B.ht_destroy(self.ctx)

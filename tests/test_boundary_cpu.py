@@ -20,17 +20,27 @@ def _built():
     build()
 
 
-def _declared():
-    text = open(os.path.join(ROOT, "include", "ht.h")).read()
+def _declared(header):
+    text = open(os.path.join(ROOT, "include", header)).read()
     return sorted(set(re.findall(r"HT_API\s+[^;(]*?\b(ht_\w+)\s*\(", text)))
 
 
 def test_library_exports_every_declared_symbol():
-    names = _declared()
+    """include/ht.h = the method's calls, include/ht_diag.h = diagnostics; the binding names exactly those."""
+    names, diag = _declared("ht.h"), _declared("ht_diag.h")
     assert len(names) >= 9 and set(names) == set(B.EXPORTS)
+    assert set(diag) == set(B.DIAG_EXPORTS) and not set(diag) & set(names)
     lib = C.CDLL(B.LIB_PATH)
-    for n in names:
+    for n in names + diag:
         assert getattr(lib, n) is not None
+
+
+def test_no_environment_variable_is_read_by_the_library():
+    """Every switch is a field of ht_tuning (read once by ht_create_ex): no getenv anywhere in the sources."""
+    csrc = os.path.join(ROOT, "paper_1507_03074_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+    assert C.sizeof(B.ht_tuning) == 64
 
 
 def test_no_torch_types_in_the_header():
@@ -54,7 +64,7 @@ def test_tables_bit_identical_to_the_oracle(bn):
 def test_query_sizes_and_argument_validation():
     cfg = B.ht_config.from_binning(WORKLOADS[2].binning, max_events=2, max_hits=5000)
     mh, ws = B.ht_query_sizes(cfg)
-    assert mh == 4 * 67_108_864 and 0 < ws < (1 << 22)
+    assert mh == 4 * 67_108_864 and 0 < ws < (1 << 22) and ws % 256 == 0
     cfg_h = B.ht_config.from_binning(WORKLOADS[1].binning, max_events=2, max_hits=100, host_slots=2, host_peak_capacity=100)
     mh1, ws1 = B.ht_query_sizes(cfg_h)
     assert ws1 > 2 * mh1

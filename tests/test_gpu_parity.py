@@ -19,12 +19,13 @@ def _oracle_batch(bn, batch):
     return [oracle_fill(bn, *batch.event(e))[0] for e in range(batch.n_events)]
 
 
-def _check_batch(bn, batch, threshold, naive=False, capacity=1 << 20, fused=True):
+def _check_batch(bn, batch, threshold, naive=False, capacity=1 << 20, fused=True, tuning=None, own_workspace=False):
     """ht_fill (or ht_fill_naive) + ht_peaks, then the fused ht_fill_peaks with and without the matrix store: all three
     against the oracle, element by element."""
     want_m = _oracle_batch(bn, batch)
     want_p = oracle_peaks_batch(bn, want_m, threshold)
-    with GpuHough(bn, max_events=max(1, batch.n_events), max_hits=batch.n_hits) as g:
+    with GpuHough(bn, max_events=max(1, batch.n_events), max_hits=batch.n_hits, tuning=tuning,
+                  own_workspace=own_workspace) as g:
         mh = g.fill(batch, naive=naive)
         got = mh_to_numpy(mh, bn, batch.n_events)
         for e in range(batch.n_events):
@@ -104,6 +105,42 @@ def test_config5_two_events_sampled():
         _, n_f, pk_f = g.fill_peaks(batch, wl.threshold, store=False)
         assert n_f == n
         np.testing.assert_array_equal(sort_peaks(pk_f, bn.cells), got_p)
+
+
+def _full_batch_both_paths(wl, n_events):
+    """ALL events of a batch workload at full size, element by element on every event, through ht_fill_peaks (one call
+    over the whole batch) and through ht_fill + ht_peaks.  The matrices stay on the device (26.8 GB / 42.9 GB per path);
+    the oracle's matrix of one event at a time is uploaded and compared there."""
+    bn = wl.binning
+    batch = generate_batch(wl, n_events=n_events)
+    cells = bn.cells
+    with GpuHough(bn, max_events=n_events, max_hits=batch.n_hits) as g:
+        mh_f, n_f, pk_f = g.fill_peaks(batch, wl.threshold)
+        mh_s = g.fill(batch)
+        n_s, pk_s = g.peaks(mh_s, n_events, wl.threshold)
+        want_p = []
+        for e in range(n_events):
+            m, _ = oracle_fill(bn, *batch.event(e))
+            want_p.append(oracle_peaks(bn, m, wl.threshold, event=e))
+            ref = torch.from_numpy(m.reshape(-1).view(np.int32)).to(g.dev)
+            assert torch.equal(mh_f[e * cells:(e + 1) * cells], ref), f"ht_fill_peaks, event {e}"
+            assert torch.equal(mh_s[e * cells:(e + 1) * cells], ref), f"ht_fill, event {e}"
+            del ref, m
+        want_p = np.concatenate(want_p)
+        assert n_f == n_s == len(want_p)
+        np.testing.assert_array_equal(sort_peaks(pk_f, cells), want_p)
+        np.testing.assert_array_equal(sort_peaks(pk_s, cells), want_p)
+    return len(want_p)
+
+
+def test_config3_all_100_events_full_size():
+    """BASELINE.json:configs[2]; "100 simulated events": every event, every cell, both call paths."""
+    assert _full_batch_both_paths(WORKLOADS[3], 100) > 10000
+
+
+def test_config5_all_10_events_full_size():
+    """BASELINE.json:configs[4]: ten 4.29 GB matrices in one call (64-bit offsets), every event, every cell."""
+    assert _full_batch_both_paths(WORKLOADS[5], 10) > 1000
 
 
 def test_naive_paper_design_matches_too():
@@ -260,6 +297,67 @@ def test_peak_capacity_overflow_and_threshold_monotonicity():
         assert n4b == n4 == len(want)
 
 
+def test_fused_kernel_list_truncation():
+    """ht_fill_peaks with a list that is too short: the count is the total, the records written are a duplicate-free
+    subset of the oracle's set; capacity 0 writes nothing; capacity == n is the whole set."""
+    wl = WORKLOADS[1]
+    bn = wl.binning
+    batch = generate_batch(wl, n_events=3)
+    want = oracle_peaks_batch(bn, _oracle_batch(bn, batch), 4)
+    full = set(map(tuple, want.tolist()))
+    assert len(want) > 7
+    with GpuHough(bn, 3, batch.n_hits) as g:
+        for store in (True, False):
+            _, n, pk = g.fill_peaks(batch, 4, capacity=7, store=store)
+            assert n == len(want) and len(pk) == 7
+            got = list(map(tuple, pk.tolist()))
+            assert all(r in full for r in got) and len(set(got)) == 7
+            _, n0, pk0 = g.fill_peaks(batch, 4, capacity=0, store=store)
+            assert n0 == len(want) and len(pk0) == 0
+            _, n1, pk1 = g.fill_peaks(batch, 4, capacity=len(want), store=store)
+            assert n1 == len(want)
+            np.testing.assert_array_equal(sort_peaks(pk1, bn.cells), want)
+            _, n2, pk2 = g.fill_peaks(batch, 4, capacity=len(want) - 1, store=store)
+            got2 = set(map(tuple, pk2.tolist()))
+            assert n2 == len(want) and len(got2) == len(want) - 1 and got2 <= full
+
+
+@pytest.mark.parametrize("tuning", [None, {"fill_batch_classification": 1}, {"fill_shared_atomics": 1}])
+def test_repeated_launches_give_the_same_bits(tuning):
+    """No timing-dependent result: 3000 back-to-back fused launches per variant (hand-rolled grid barrier, named-barrier
+    pipeline, TMA proxy fence, dependent launches overlapping their predecessor's tail), matrix and peak set compared on
+    the device after every launch against a reference that is itself checked against the oracle."""
+    wl = WORKLOADS[2]
+    bn = Binning(4, 16, 256, 256)
+    batch = generate_batch(wl, n_events=1)
+    want_m = _oracle_batch(bn, batch)[0]
+    want_p = oracle_peaks(bn, want_m, wl.threshold)
+    cap = 1 << 13
+    with GpuHough(bn, 1, batch.n_hits, tuning=tuning) as g:
+        dx, dy, dz, doff = g.upload(batch)
+        ref_m = torch.from_numpy(want_m.reshape(-1).view(np.int32)).to(g.dev)
+        ref_cells = torch.from_numpy(want_p["cell"].astype(np.int64)).to(g.dev)
+        ref_counts = torch.from_numpy(want_p["count"].astype(np.int64)).to(g.dev)
+        mhs = [torch.empty(bn.cells, dtype=torch.int32, device=g.dev) for _ in range(2)]
+        outs = [torch.zeros(3 * cap, dtype=torch.int32, device=g.dev) for _ in range(2)]
+        nfs = [torch.zeros(1, dtype=torch.int32, device=g.dev) for _ in range(2)]
+        bad = torch.zeros(1, dtype=torch.int64, device=g.dev)
+        n = len(want_p)
+        for it in range(3000):
+            k = it & 1
+            B.ht_fill_peaks(g.ctx, dx, dy, dz, doff, 1, batch.n_hits, mhs[k], wl.threshold, outs[k], cap, nfs[k], None)
+            if it >= 1:                                             # check the PREVIOUS launch while this one runs behind it
+                j = k ^ 1
+                rec = outs[j][:3 * n].view(n, 3).to(torch.int64)
+                order = torch.argsort(rec[:, 1])
+                ok = (torch.equal(mhs[j], ref_m) & torch.equal(rec[order, 1], ref_cells) &
+                      torch.equal(rec[order, 2], ref_counts) & (int(nfs[j].item()) == n))
+                if not ok:
+                    bad += 1
+        torch.cuda.synchronize()
+        assert int(bad.item()) == 0
+
+
 # ------------------------------------------------------------------ streams, repeated calls, host entry point
 def test_fill_on_a_side_stream_and_buffer_reuse():
     wl = WORKLOADS[1]
@@ -294,6 +392,53 @@ def test_run_host_end_to_end():
         assert B.ht_kernel_launches(g.ctx) >= 2 * 3            # 2 calls x 3 groups of <= 2 events, one fused kernel each
 
 
+def test_submit_wait_host_pipeline():
+    """ht_submit_host / ht_wait_host: events in flight in several slots, waited for out of submission order, slots
+    reused, misuse refused; every event's peak list against the oracle."""
+    wl = WORKLOADS[2]
+    bn = Binning(4, 16, 256, 256)
+    events = [generate_batch(wl, n_events=1, first_event=e) for e in range(7)]
+    wants = [oracle_peaks(bn, oracle_fill(bn, *b.event(0))[0], wl.threshold) for b in events]
+    for tuning in (None, {"host_copy_input": 1}):
+        with GpuHough(bn, 1, 6000, host_slots=3, host_peak_capacity=4096, tuning=tuning) as g:
+            out = np.zeros(4096, B.PEAK_DTYPE)
+            in_flight = {}
+            order = []
+            for k, b in enumerate(events):
+                slot = k % 3
+                if slot in in_flight:
+                    kk = in_flight.pop(slot)
+                    n = B.ht_wait_host(g.ctx, slot, out, 4096)
+                    assert n == len(wants[kk])
+                    np.testing.assert_array_equal(sort_peaks(out[:n], bn.cells), wants[kk])
+                    order.append(kk)
+                B.ht_submit_host(g.ctx, slot, b.x, b.y, b.z, b.n_hits, wl.threshold)
+                in_flight[slot] = k
+                with pytest.raises(B.HtError):                       # the slot is busy
+                    B.ht_submit_host(g.ctx, slot, b.x, b.y, b.z, b.n_hits, wl.threshold)
+            with pytest.raises(B.HtError):                           # events in flight: the synchronous call is refused
+                B.ht_run_host(g.ctx, events[0].x, events[0].y, events[0].z, events[0].event_offsets, 1, events[0].n_hits,
+                              wl.threshold, out, 4096)
+            for slot in sorted(in_flight, reverse=True):             # not the submission order
+                kk = in_flight[slot]
+                n = B.ht_wait_host(g.ctx, slot, out, 4096)
+                assert n == len(wants[kk])
+                np.testing.assert_array_equal(sort_peaks(out[:n], bn.cells), wants[kk])
+                order.append(kk)
+            assert sorted(order) == list(range(7))
+            with pytest.raises(B.HtError):                           # nothing submitted
+                B.ht_wait_host(g.ctx, 0, out, 4096)
+            # truncated read-back: the count is the total, the records a subset
+            B.ht_submit_host(g.ctx, 1, events[2].x, events[2].y, events[2].z, events[2].n_hits, wl.threshold)
+            small = np.zeros(5, B.PEAK_DTYPE)
+            n = B.ht_wait_host(g.ctx, 1, small, 5)
+            full = set(map(tuple, wants[2].tolist()))
+            assert n == len(wants[2]) and all(tuple(r) in full for r in small.tolist())
+            # a device-pointer call on another stream right after the host calls (ordered by the library)
+            m = g.fill(events[3])
+            np.testing.assert_array_equal(mh_to_numpy(m, bn, 1)[0], oracle_fill(bn, *events[3].event(0))[0])
+
+
 def test_error_codes_on_device_calls():
     bn = WORKLOADS[1].binning
     batch = generate_batch(1)
@@ -317,22 +462,46 @@ def test_error_codes_on_device_calls():
 
 
 # ------------------------------------------------------------------ every code path of the fill kernel
-@pytest.mark.parametrize("env", [{"HT_FILL_MODE": "0"},            # batch classification (global buckets) on single events too
-                                 {"HT_FILL_HIT_CAP": "32"},         # most hits bypass the shared-memory staging
-                                 {"HT_FILL_SLAB_KB": "8"},          # many small tiles, rows shared by few warps
-                                 {"HT_FILL_NO_BULK": "1"},          # plain stores instead of the TMA
-                                 {"HT_FILL_MODE": "0", "HT_FILL_HIT_CAP": "0"}])
-def test_fill_kernel_variants_are_bit_exact(env, monkeypatch):
-    """The launch-time switches of the fill kernel (read from the environment at every call) change how the work is
-    organised, never the result."""
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
+@pytest.mark.parametrize("tuning", [{"fill_batch_classification": 1},   # batch classification (global buckets) on single events too
+                                    {"fill_hit_cap": 32},                # most hits bypass the shared-memory staging
+                                    {"fill_slab_kb": 8},                 # many small tiles, rows shared by few warps
+                                    {"fill_plain_stores": 1},            # plain stores instead of the TMA
+                                    {"fill_batch_classification": 1, "fill_hit_cap": -1},
+                                    {"fill_shared_atomics": 1},          # votes as shared-memory atomics
+                                    {"fill_shared_atomics": 1, "fill_hit_cap": -1},
+                                    {"cooperative_launch": 1},           # cudaLaunchCooperativeKernel instead of the dependent launch
+                                    {"peaks_unroll": 4}, {"peaks_unroll": 8, "peaks_ctas_per_sm": 2}])
+def test_fill_kernel_variants_are_bit_exact(tuning):
+    """The switches of ht_tuning (read once by ht_create_ex) change how the work is organised, never the result."""
     wl = WORKLOADS[2]
     bn = Binning(4, 16, 256, 512)                                   # 33.5 M cells: the oracle takes a fraction of a second
     one = generate_batch(wl, n_events=1)
-    assert _check_batch(bn, one, wl.threshold) > 0
+    assert _check_batch(bn, one, wl.threshold, tuning=tuning) > 0
     three = generate_batch(WORKLOADS[3], n_events=3)
-    assert _check_batch(bn, three, wl.threshold) > 0
+    assert _check_batch(bn, three, wl.threshold, tuning=tuning, own_workspace=True) > 0
+
+
+def test_caller_owned_workspace_and_bad_tuning():
+    """ht_query_sizes -> caller allocates -> ht_create_ex: same results; a workspace that is too small or misaligned and
+    a tuning block with unknown fields set are refused."""
+    wl = WORKLOADS[1]
+    bn = wl.binning
+    batch = generate_batch(wl, n_events=2)
+    assert _check_batch(bn, batch, wl.threshold, own_workspace=True) > 0
+    cfg = B.ht_config.from_binning(bn, max_events=2, max_hits=batch.n_hits, device=0)
+    nbytes = B.ht_query_sizes(cfg)[1]
+    ws = torch.empty(nbytes + 512, dtype=torch.uint8, device="cuda")
+    base = (ws.data_ptr() + 255) // 256 * 256
+    for args in ((base, nbytes - 1), (base + 4, nbytes)):
+        with pytest.raises(B.HtError) as ei:
+            B.ht_create_ex(cfg, None, *args)
+        assert ei.value.status == B.HT_ERR_INVALID_ARG
+    bad = B.ht_tuning()
+    bad.reserved[3] = 1
+    with pytest.raises(B.HtError):
+        B.ht_create_ex(cfg, bad)
+    with pytest.raises(B.HtError):
+        B.ht_create_ex(cfg, B.ht_tuning(peaks_unroll=3))
 
 
 def test_dense_tiles_with_many_peak_candidates():
@@ -352,14 +521,13 @@ def test_division_shortcut_equals_fdiv_rn_on_four_billion_pairs():
     assert B.ht_selftest_division(0, 100_000_000, 987654321) == 0
 
 
-@pytest.mark.parametrize("zero_copy", ["1", "0"])
-def test_run_host_single_event_zero_copy_and_copy(zero_copy, monkeypatch):
+@pytest.mark.parametrize("copy_input", [0, 1])
+def test_run_host_single_event_zero_copy_and_copy(copy_input):
     """One event through ht_run_host: the kernel reads the hits straight from the pinned block (default) or the block is
     copied to the device first; same matrix, same peaks, several calls in a row on one context."""
-    monkeypatch.setenv("HT_HOST_ZERO_COPY", zero_copy)
     wl = WORKLOADS[2]
     bn = Binning(4, 16, 256, 256)
-    with GpuHough(bn, 1, 6000, host_slots=1, host_peak_capacity=8192) as g:
+    with GpuHough(bn, 1, 6000, host_slots=1, host_peak_capacity=8192, tuning={"host_copy_input": copy_input}) as g:
         for ev in range(3):
             batch = generate_batch(wl, n_events=1, first_event=ev)
             want_m = _oracle_batch(bn, batch)
