@@ -98,16 +98,14 @@ typedef struct ht_peak {
 typedef struct ht_tuning {
     int32_t fill_batch_classification; /* 1: classify through global buckets (the batch path) also for single events */
     int32_t fill_slab_kb;              /* > 0: cap of one shared-memory slab in KB (0: as large as fits) */
-    int32_t fill_hit_cap;              /* > 0: hits of a tile staged in shared memory at most; -1: none (0: default) */
     int32_t fill_plain_stores;         /* 1: tiles leave with plain stores instead of bulk (TMA) stores */
-    int32_t fill_shared_atomics;       /* 1: votes are shared-memory atomics (0: warp-private read-modify-write) */
     int32_t cooperative_launch;        /* 1: cudaLaunchCooperativeKernel (0: ordinary launch, programmatic dependent
                                           launch: the next call's prologue overlaps this call's tail) */
     int32_t host_copy_input;           /* 1: ht_run_host / ht_submit_host copy the hits to the device (0: single events
                                           are read by the kernel straight from the pinned block, zero-copy) */
     int32_t peaks_unroll;              /* 2, 4 or 8 independent 16-byte loads per thread of the peak scan (0: 2) */
     int32_t peaks_ctas_per_sm;         /* > 0: cap of the peak scan's resident CTAs per SM */
-    int32_t reserved[7];               /* must be zero */
+    int32_t reserved[9];               /* must be zero */
 } ht_tuning;
 
 /* Sizes implied by a configuration: bytes of one event's matrix, and bytes of the context's device workspace

@@ -349,3 +349,95 @@ int64_t oracle_merge_ridges(const oracle_binning *g, const oracle_peak *peaks, i
     free(all);
     return found;
 }
+
+/*
+ * Truth matching of track candidates (SPEC.md section 6, reading R20; SURVEY.md section 8(f) f3 "truth-matched
+ * efficiency / fake rate / resolution on the synthetic events"; the stand-in for PAPER.md:29-33, Fig. 1, where "the
+ * rho = sqrt(A^2+B^2) and phi = tan^-1(B/A) are shown together with the corresponding resolutions").
+ * A candidate stands for the circle through the origin whose centre (A_c, B_c) is the centre of its cell (section 4);
+ * a generated track IS such a circle with centre (A_t, B_t) (generator G3).  All arithmetic in binary64, one rounding
+ * per operation, in the order written; no arctangent enters a decision:
+ *   rho_c = sqrt(A_c*A_c + B_c*B_c), rho_t alike
+ *   compatible(c, t)  <=>  same event  and  |rho_c - rho_t| <= w_rho  and  A_c*A_t + B_c*B_t >= cos_w_phi * (rho_c*rho_t)
+ *   d2(c, t) = (A_c-A_t)^2 + (B_c-B_t)^2
+ *   cand_match[c]  = the compatible t of smallest d2 (ties: smallest index t), or -1: the candidate is a FAKE
+ *   truth_match[t] = among the c with cand_match[c] == t the one of smallest d2 (ties: smallest cell), or -1: NOT FOUND;
+ *                    the other candidates matched to t are DUPLICATES
+ *   residuals of a found track, with c = truth_match[t]: d_rho = rho_c - rho_t, d_phi = atan2(A_t*B_c - B_t*A_c, A_c*A_t + B_c*B_t)
+ * Returns 0, or -1 on bad arguments.  Pins: P16 (noiseless tracks through generator, fill, peaks, merge: all found, no
+ * fake, residuals below one cell diagonal), P17 (a soft track split by a sector edge is not found), P18 (hand-built
+ * lists), P19 (invariants, and a brute force in polar coordinates away from the window edges).
+ */
+typedef struct { uint32_t event, pad; double a, b; } oracle_truth;
+typedef struct {
+    int64_t n_cand, n_truth, n_matched, n_fake, n_found, n_duplicate;
+    double sum_drho, sum_drho2, sum_dphi, sum_dphi2;        /* over the found tracks */
+} oracle_match_summary;
+
+int oracle_match_truth(const oracle_binning *g, const oracle_merged *cand, int64_t n_cand, const oracle_truth *truth,
+                       int64_t n_truth, double w_rho, double cos_w_phi, int32_t *cand_match, int32_t *truth_match,
+                       oracle_match_summary *sum)
+{
+    if (!binning_ok(g) || n_cand < 0 || n_truth < 0 || !sum) return -1;
+    if ((n_cand > 0 && (!cand || !cand_match)) || (n_truth > 0 && (!truth || !truth_match))) return -1;
+    if (!(w_rho >= 0.0) || !(cos_w_phi >= -1.0 && cos_w_phi <= 1.0)) return -1;
+    const float dA = (g->a_max - g->a_min) / (float)g->n_a;
+    const float dB = (g->b_max - g->b_min) / (float)g->n_b;
+    const uint64_t cells = (uint64_t)g->n_theta * g->n_phi * g->n_a * g->n_b;
+    double *best_d2 = (double *)malloc(sizeof(double) * (size_t)(n_truth + 1));
+    if (!best_d2) return -1;
+    for (int64_t t = 0; t < n_truth; ++t) truth_match[t] = -1;
+    memset(sum, 0, sizeof *sum);
+    sum->n_cand = n_cand;
+    sum->n_truth = n_truth;
+    for (int64_t c = 0; c < n_cand; ++c) {
+        if (cand[c].cell >= cells) { free(best_d2); return -1; }
+        const uint32_t ib = cand[c].cell % (uint32_t)g->n_b;
+        const uint32_t ia = (cand[c].cell / (uint32_t)g->n_b) % (uint32_t)g->n_a;
+        const float fa = (float)ia + 0.5f, fb = (float)ib + 0.5f;
+        const float pa = fa * dA, pb = fb * dB;
+        const float Af = g->a_min + pa, Bf = g->b_min + pb;            /* bin centres (R5, R18), binary32 as in section 4 */
+        const double Ac = (double)Af, Bc = (double)Bf;
+        const double rho_c = sqrt(Ac * Ac + Bc * Bc);
+        int64_t best = -1;
+        double best_c = 0.0;
+        for (int64_t t = 0; t < n_truth; ++t) {
+            if (truth[t].event != cand[c].event) continue;
+            const double At = truth[t].a, Bt = truth[t].b;
+            const double rho_t = sqrt(At * At + Bt * Bt);
+            const double dr = rho_c - rho_t;
+            if (!(fabs(dr) <= w_rho)) continue;
+            const double dot = Ac * At + Bc * Bt;
+            if (!(dot >= cos_w_phi * (rho_c * rho_t))) continue;
+            const double ea = Ac - At, eb = Bc - Bt;
+            const double d2 = ea * ea + eb * eb;
+            if (best < 0 || d2 < best_c) { best = t; best_c = d2; }
+        }
+        cand_match[c] = (int32_t)best;
+        if (best < 0) { ++sum->n_fake; continue; }
+        ++sum->n_matched;
+        const int32_t cur = truth_match[best];
+        if (cur < 0 || best_c < best_d2[best] || (best_c == best_d2[best] && cand[c].cell < cand[cur].cell)) {
+            truth_match[best] = (int32_t)c;
+            best_d2[best] = best_c;
+        }
+    }
+    for (int64_t t = 0; t < n_truth; ++t) {
+        const int32_t c = truth_match[t];
+        if (c < 0) continue;
+        ++sum->n_found;
+        const uint32_t ib = cand[c].cell % (uint32_t)g->n_b;
+        const uint32_t ia = (cand[c].cell / (uint32_t)g->n_b) % (uint32_t)g->n_a;
+        const float fa = (float)ia + 0.5f, fb = (float)ib + 0.5f;
+        const float pa = fa * dA, pb = fb * dB;
+        const float Af = g->a_min + pa, Bf = g->b_min + pb;
+        const double Ac = (double)Af, Bc = (double)Bf, At = truth[t].a, Bt = truth[t].b;
+        const double dr = sqrt(Ac * Ac + Bc * Bc) - sqrt(At * At + Bt * Bt);
+        const double dp = atan2(At * Bc - Bt * Ac, Ac * At + Bc * Bt);
+        sum->sum_drho += dr; sum->sum_drho2 += dr * dr;
+        sum->sum_dphi += dp; sum->sum_dphi2 += dp * dp;
+    }
+    sum->n_duplicate = sum->n_matched - sum->n_found;
+    free(best_d2);
+    return 0;
+}

@@ -13,6 +13,16 @@ from .build import build
 PEAK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32)])
 MERGED_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32), ("n_peaks", np.uint32),
                          ("rho", np.float64), ("phi", np.float64)])                       # == oracle_merged
+TRUTH_DTYPE = np.dtype([("event", np.uint32), ("pad", np.uint32), ("a", np.float64), ("b", np.float64)])   # == oracle_truth
+
+
+class MatchSummary(C.Structure):                                                                 # == oracle_match_summary
+    _fields_ = [("n_cand", C.c_int64), ("n_truth", C.c_int64), ("n_matched", C.c_int64), ("n_fake", C.c_int64),
+                ("n_found", C.c_int64), ("n_duplicate", C.c_int64), ("sum_drho", C.c_double), ("sum_drho2", C.c_double),
+                ("sum_dphi", C.c_double), ("sum_dphi2", C.c_double)]
+
+    def as_dict(self) -> dict:
+        return {name: getattr(self, name) for name, _ in self._fields_}
 
 
 class OracleBinning(C.Structure):
@@ -60,6 +70,10 @@ def _load():
         lib.oracle_merge_ridges.restype = C.c_int64
         lib.oracle_merge_ridges.argtypes = [C.POINTER(OracleBinning), C.c_void_p, C.c_int64, C.c_uint32, C.c_void_p,
                                             C.c_int64]
+        lib.oracle_match_truth.restype = C.c_int
+        lib.oracle_match_truth.argtypes = [C.POINTER(OracleBinning), C.c_void_p, C.c_int64, C.c_void_p, C.c_int64,
+                                           C.c_double, C.c_double, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
+                                           C.POINTER(MatchSummary)]
         _lib = lib
     return _lib
 
@@ -173,3 +187,19 @@ def oracle_merge_ridges(binning, peaks: np.ndarray, window: int) -> np.ndarray:
     if n < 0:
         raise ValueError("oracle_merge_ridges: invalid arguments")
     return out[:n]
+
+
+def oracle_match_truth(binning, candidates: np.ndarray, truth: np.ndarray, w_rho: float, cos_w_phi: float):
+    """Truth matching (SPEC.md section 6, R20): (cand_match[n_cand], truth_match[n_truth], summary dict).
+    ``candidates``: MERGED_DTYPE records; ``truth``: TRUTH_DTYPE records (event, centre a, b in mm)."""
+    g = OracleBinning.of(binning)
+    cd = np.ascontiguousarray(candidates, dtype=MERGED_DTYPE)
+    tr = np.ascontiguousarray(truth, dtype=TRUTH_DTYPE)
+    cm, tm = np.empty(len(cd), np.int32), np.empty(len(tr), np.int32)
+    s = MatchSummary()
+    ip = C.POINTER(C.c_int32)
+    if _load().oracle_match_truth(C.byref(g), cd.ctypes.data_as(C.c_void_p), len(cd), tr.ctypes.data_as(C.c_void_p), len(tr),
+                                  float(w_rho), float(cos_w_phi), cm.ctypes.data_as(ip), tm.ctypes.data_as(ip),
+                                  C.byref(s)) != 0:
+        raise ValueError("oracle_match_truth: invalid arguments")
+    return cm, tm, s.as_dict()

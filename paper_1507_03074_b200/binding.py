@@ -53,10 +53,10 @@ class ht_config(C.Structure):
 
 class ht_tuning(C.Structure):
     """How the work is organised on the device (include/ht.h); never changes a result.  All zero = defaults."""
-    _fields_ = [("fill_batch_classification", C.c_int32), ("fill_slab_kb", C.c_int32), ("fill_hit_cap", C.c_int32),
-                ("fill_plain_stores", C.c_int32), ("fill_shared_atomics", C.c_int32), ("cooperative_launch", C.c_int32),
+    _fields_ = [("fill_batch_classification", C.c_int32), ("fill_slab_kb", C.c_int32),
+                ("fill_plain_stores", C.c_int32), ("cooperative_launch", C.c_int32),
                 ("host_copy_input", C.c_int32), ("peaks_unroll", C.c_int32), ("peaks_ctas_per_sm", C.c_int32),
-                ("reserved", C.c_int32 * 7)]
+                ("reserved", C.c_int32 * 9)]
 
 
 class HtError(RuntimeError):

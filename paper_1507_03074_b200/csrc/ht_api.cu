@@ -116,13 +116,15 @@ void build_tables(const ht_config *c, float *two_a, float *tth, float *pph, floa
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+constexpr size_t kBucketBytesMax = 32u << 20;   // cap of the single-event bucket region (bigger events take the batch path)
 constexpr size_t kResHeader = 16;      // result block: [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
 
 // Layout of the context's device workspace (one contiguous block: caller-owned or allocated by ht_create) and sizes of
 // the pinned host staging blocks.  Offsets are multiples of 256.
 struct WorkspaceLayout {
-    size_t tables, counters, hits, bucket_start, counts, in_dev, mh;      // offsets
+    size_t tables, counters, hits, buckets, bucket_start, counts, in_dev, mh;      // offsets
     size_t hits_part;             // bytes of one of the 6 per-hit arrays
+    size_t buckets_bytes;         // single-event classification: P buckets of n_hits records each (as far as this holds them)
     size_t in_block, res_block;   // bytes of ONE slot's input block [offsets | x | y | z] and result block
     size_t total;
 };
@@ -138,6 +140,8 @@ WorkspaceLayout workspace_layout(const ht_config *c)
     w.counters = take(256);
     w.hits_part = align_up(sizeof(float) * (size_t)c->max_hits, 256);
     w.hits = take(6 * w.hits_part);            // hit records (4 words per hit), h_plane, h_rel
+    w.buckets_bytes = std::min<size_t>(planes_all * align_up((size_t)c->max_hits, 4) * 16u, kBucketBytesMax);
+    w.buckets = take(w.buckets_bytes);
     w.bucket_start = take(sizeof(int32_t) * (size_t)c->max_events * (planes_all + 1));
     w.counts = take(sizeof(uint32_t) * (size_t)c->max_events * planes_all);
     if (c->host_slots > 0) {
@@ -155,7 +159,7 @@ WorkspaceLayout workspace_layout(const ht_config *c)
 // tables, the staged hits and -- in mode 1 -- the plane offsets and the uint16 hit index fit the CTA's shared memory.
 struct FillPlan {
     bool ok = false;
-    int mode = 0, rows_slab = 0, hit_cap = 0;
+    int mode = 0, rows_slab = 0;
     uint32_t slab_words = 0;
     size_t smem = 0;
 };
@@ -182,11 +186,11 @@ struct ht_ctx {
     float *d_tth = nullptr, *d_pph = nullptr;
     uint32_t *d_counters = nullptr;
     // hit buckets written by the fill kernel's prologue (a0): per-hit vote constants grouped by (event, plane)
-    float *d_bx = nullptr, *d_br2 = nullptr, *d_bden = nullptr;
+    float *d_bx = nullptr;                 // mode 0: [max_hits] records
+    float *d_buckets = nullptr;            // mode 1: [P][n_hits] records
     int32_t *d_hplane = nullptr, *d_hrel = nullptr;   // [max_hits] phase-1 spill
     int32_t *d_bucket_start = nullptr;     // [max_events * (P+1)]
     uint32_t *d_counts = nullptr;          // [max_events * P], zero between calls
-    uint32_t bar_epoch = 0;                // host mirror of the barrier counter that only grows (d_counters[5])
     bool fill_ok = false;
     size_t fill_smem_max[2] = {0, 0};      // dynamic shared memory budget: [0] ht_fill, [1] fused peaks
     FillPlan plan_cache[2];
@@ -212,8 +216,8 @@ size_t fill_smem_bytes(const ht_config &c, long long rows, int mode, long long n
 {
     const size_t slab = align_up((size_t)rows * (size_t)c.n_b * 4u, 16);
     size_t b = 2u * slab + 8u * 4u * (size_t)(rows + 4);     // two slabs, two_a[8 ring entries][rows + 4]
-    b += align_up(4u * ((size_t)c.n_theta * (size_t)c.n_phi + 1u), 16);      // plane offsets, padded: the staged hits are float4
-    if (mode == 1) b += 2u * (size_t)n_hits;
+    if (mode == 1) b += 4u * (size_t)c.n_theta * (size_t)c.n_phi;            // hits per plane
+    (void)n_hits;
     return align_up(b, 16);
 }
 
@@ -281,7 +285,7 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
         for (int32_t r : tun.reserved)
             if (r != 0) return HT_ERR_INVALID_ARG;
         if (tun.peaks_unroll != 0 && tun.peaks_unroll != 2 && tun.peaks_unroll != 4 && tun.peaks_unroll != 8) return HT_ERR_INVALID_ARG;
-        if (tun.fill_slab_kb < 0 || tun.fill_hit_cap < -1 || tun.peaks_ctas_per_sm < 0) return HT_ERR_INVALID_ARG;
+        if (tun.fill_slab_kb < 0 || tun.peaks_ctas_per_sm < 0) return HT_ERR_INVALID_ARG;
     }
     const WorkspaceLayout lay = workspace_layout(cfg);
     if (d_workspace && (workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0)) return HT_ERR_INVALID_ARG;
@@ -327,8 +331,7 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
     ctx->d_pph = ctx->d_tth + (cfg->n_theta + 1);
     ctx->d_counters = reinterpret_cast<uint32_t *>(ws + lay.counters);
     ctx->d_bx = reinterpret_cast<float *>(ws + lay.hits);
-    ctx->d_br2 = reinterpret_cast<float *>(ws + lay.hits + lay.hits_part);
-    ctx->d_bden = reinterpret_cast<float *>(ws + lay.hits + 2 * lay.hits_part);
+    ctx->d_buckets = reinterpret_cast<float *>(ws + lay.buckets);
     ctx->d_hplane = reinterpret_cast<int32_t *>(ws + lay.hits + 4 * lay.hits_part);
     ctx->d_hrel = reinterpret_cast<int32_t *>(ws + lay.hits + 5 * lay.hits_part);
     ctx->d_bucket_start = reinterpret_cast<int32_t *>(ws + lay.bucket_start);
@@ -426,18 +429,14 @@ FillPlan compute_fill_plan(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, 
     const size_t budget_all = ctx->fill_smem_max[peaks ? 1 : 0];
     const size_t row_bytes = (size_t)c.n_b * 4u;
     const long long planes = (long long)c.n_theta * c.n_phi;
-    // mode 1 (per-CTA shared-memory hit index): one event, uint16 indices and plane ids, an index of at most 48 KB
-    int mode = (n_events == 1 && n_hits <= 24576 && planes < 65535 && !tun.fill_batch_classification) ? 1 : 0;
+    // mode 1 (one-pass classification into fixed-capacity plane buckets): one event whose P x n_hits records fit the region
+    int mode = (n_events == 1 && (size_t)planes * align_up((size_t)n_hits, 4) * 16u <= ctx->lay.buckets_bytes &&
+                planes * 4 < 32768 && !tun.fill_batch_classification) ? 1 : 0;
     // without the fused peak search the kernel is purely store-bound and measured fastest with slabs of <= 96 KB
     // (config 2, B200: 51.5 us at 96 KB, 53.4 at 100 KB, 59.4 at 104 KB); with it, the largest slab wins (fewer halo rows)
     const int slab_kb = tun.fill_slab_kb > 0 ? tun.fill_slab_kb : (peaks ? 0 : 96);
-    // shared memory set aside for the hits staged per tile (two buffers of 16 bytes per hit): room for twice the
-    // average number of hits per (event, plane), at most 512 hits; whatever else is left over is added below
-    long long want_cap = 2ll * (long long)n_hits / ((long long)(n_events > 0 ? n_events : 1) * planes);
-    want_cap = (want_cap + 31) / 32 * 32;
-    want_cap = std::min(512ll, std::max(32ll, want_cap));
     auto rows_for = [&](int md) -> long long {
-        const size_t budget = budget_all > (size_t)want_cap * 32u ? budget_all - (size_t)want_cap * 32u : 0;
+        const size_t budget = budget_all;
         long long rows = c.n_a;
         if (slab_kb > 0 && rows > (long long)((size_t)slab_kb * 1024u / row_bytes)) rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
         if (rows < 1) rows = 1;
@@ -449,9 +448,6 @@ FillPlan compute_fill_plan(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, 
             }
             rows = lo;
         }
-        // mode 1 sorts in the slab space: plane id + slot, 4 bytes per hit, and a copy of the angle tables
-        if (md == 1 && 4u * (size_t)n_hits + 4u * (size_t)(c.n_theta + c.n_phi + 4) >
-                           2u * align_up((size_t)rows * row_bytes, 16)) return 0;
         return rows;
     };
     for (;; mode = 0) {
@@ -462,13 +458,6 @@ FillPlan compute_fill_plan(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, 
             pl.rows_slab = (int)rows;
             pl.slab_words = (uint32_t)(align_up((size_t)rows * row_bytes, 16) / 4u);
             pl.smem = fill_smem_bytes(c, rows, mode, n_hits);
-            // what is left of the budget stages the hits of two tiles (x, r2, den, rc: 16 bytes per hit), up to 512 per tile
-            long long cap = ((long long)(budget_all - pl.smem) / 32) / 32 * 32;
-            cap = std::min(cap, 512ll);
-            if (tun.fill_hit_cap > 0) cap = std::min(cap, (long long)tun.fill_hit_cap / 32 * 32);
-            if (tun.fill_hit_cap < 0) cap = 0;
-            pl.hit_cap = (int)cap;
-            pl.smem += (size_t)cap * 32u;
             return pl;
         }
         if (mode == 0) return pl;                                              // one row does not fit: ht_fill_naive only
@@ -500,9 +489,9 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.x = d_x; a.y = d_y; a.z = d_z; a.event_offsets = d_off; a.n_events = n_events; a.n_hits = n_hits_total;
     a.tth = ctx->d_tth; a.pph = ctx->d_pph;
     a.mode = pl.mode;
-    a.hit_cap = pl.hit_cap;
     a.counts = ctx->d_counts; a.bucket_start = ctx->d_bucket_start; a.h_plane = ctx->d_hplane; a.h_rel = ctx->d_hrel;
-    a.bx = ctx->d_bx; a.br2 = ctx->d_br2; a.bden = ctx->d_bden;
+    a.bx = pl.mode == 1 ? ctx->d_buckets : ctx->d_bx;
+    a.bucket_cap = (int)align_up((size_t)n_hits_total, 4);
     a.bar = ctx->d_counters + 2;
     a.g = g;
     a.rows_slab = pl.rows_slab;
@@ -523,7 +512,6 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.n_tiles = (uint32_t)n_tiles;
     a.mh = d_mh;
     a.bulk_ok = (g.n_b % 4 == 0) && ((reinterpret_cast<uintptr_t>(d_mh) & 15u) == 0) && !ctx->tun.fill_plain_stores;
-    a.atomic_votes = ctx->tun.fill_shared_atomics ? 1 : 0;
     a.early_inputs = early_inputs ? 1 : 0;
     a.threshold = threshold;
     static_assert(sizeof(ht::PeakOut) == sizeof(ht_peak), "peak record layout");
@@ -537,14 +525,10 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     if (grid < 1) grid = 1;
     const int ro = order_after_previous(ctx, st);
     if (ro != HT_OK) return ro;
-    // Mode 1's grid barrier: the fast one-shot form needs the host to know the counter's value, which a launch captured
-    // into a CUDA graph (replayed any number of times) cannot; captured launches use the self-resetting barrier.
-    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-    HT_CUDA(cudaStreamIsCapturing(st, &cap));
-    const bool one_shot = pl.mode == 1 && cap == cudaStreamCaptureStatusNone;
+    // the kernel leaves every counter it uses at zero (its last CTA resets them): nothing here depends on host-side state,
+    // so the launch can be captured into a CUDA graph and replayed
     a.tile_counter = ctx->d_counters + 6;
-    a.bar_count = one_shot ? ctx->d_counters + 5 : nullptr;
-    a.bar_target = ctx->bar_epoch + (uint32_t)grid;
+    a.bar_count = ctx->d_counters + 5;
     const void *fn = peaks ? reinterpret_cast<const void *>(ht::fill_tiles_kernel<true>)
                            : reinterpret_cast<const void *>(ht::fill_tiles_kernel<false>);
     void *params[] = {&a};
@@ -566,7 +550,6 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
         lc.numAttrs = 1;
         HT_CUDA(cudaLaunchKernelExC(&lc, fn, params));
     }
-    if (one_shot) ctx->bar_epoch = a.bar_target;
     ++ctx->launches;
     ctx->info[0] = (int32_t)grid; ctx->info[1] = ht::kFillThreads; ctx->info[2] = (int32_t)pl.smem;
     ctx->info[3] = rows_store; ctx->info[7] = pl.mode;
@@ -936,6 +919,21 @@ int ht_diag_vote_rates(int32_t device, int32_t iters, double *h_rates, uint64_t 
     *h_sum_errors = errors;
     return HT_OK;
 }
+
+#ifdef HT_PROFILE_PHASES
+// build-time instrumentation only: copy (and clear) the per-CTA phase counters of the fill kernel
+__attribute__((visibility("default"))) int ht_prof_read(uint64_t *h_out, int32_t n_words, int32_t reset)
+{
+    if (!h_out || n_words < 0 || n_words > 256 * 16) return HT_ERR_INVALID_ARG;
+    HT_CUDA(cudaDeviceSynchronize());
+    HT_CUDA(cudaMemcpyFromSymbol(h_out, ht::g_prof, sizeof(uint64_t) * (size_t)n_words));
+    if (reset) {
+        static const unsigned long long zeros[256 * 16] = {};
+        HT_CUDA(cudaMemcpyToSymbol(ht::g_prof, zeros, sizeof zeros));
+    }
+    return HT_OK;
+}
+#endif
 
 int64_t ht_kernel_launches(const ht_ctx *ctx) { return ctx ? ctx->launches : 0; }
 

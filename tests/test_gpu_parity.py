@@ -322,7 +322,7 @@ def test_fused_kernel_list_truncation():
             assert n2 == len(want) and len(got2) == len(want) - 1 and got2 <= full
 
 
-@pytest.mark.parametrize("tuning", [None, {"fill_batch_classification": 1}, {"fill_shared_atomics": 1}])
+@pytest.mark.parametrize("tuning", [None, {"fill_batch_classification": 1}, {"cooperative_launch": 1}])
 def test_repeated_launches_give_the_same_bits(tuning):
     """No timing-dependent result: 3000 back-to-back fused launches per variant (hand-rolled grid barrier, named-barrier
     pipeline, TMA proxy fence, dependent launches overlapping their predecessor's tail), matrix and peak set compared on
@@ -463,12 +463,9 @@ def test_error_codes_on_device_calls():
 
 # ------------------------------------------------------------------ every code path of the fill kernel
 @pytest.mark.parametrize("tuning", [{"fill_batch_classification": 1},   # batch classification (global buckets) on single events too
-                                    {"fill_hit_cap": 32},                # most hits bypass the shared-memory staging
                                     {"fill_slab_kb": 8},                 # many small tiles, rows shared by few warps
                                     {"fill_plain_stores": 1},            # plain stores instead of the TMA
-                                    {"fill_batch_classification": 1, "fill_hit_cap": -1},
-                                    {"fill_shared_atomics": 1},          # votes as shared-memory atomics
-                                    {"fill_shared_atomics": 1, "fill_hit_cap": -1},
+                                    {"fill_batch_classification": 1, "fill_slab_kb": 8},
                                     {"cooperative_launch": 1},           # cudaLaunchCooperativeKernel instead of the dependent launch
                                     {"peaks_unroll": 4}, {"peaks_unroll": 8, "peaks_ctas_per_sm": 2}])
 def test_fill_kernel_variants_are_bit_exact(tuning):
