@@ -105,7 +105,9 @@ typedef struct ht_tuning {
                                           are read by the kernel straight from the pinned block, zero-copy) */
     int32_t peaks_unroll;              /* 2, 4 or 8 independent 16-byte loads per thread of the peak scan (0: 2) */
     int32_t peaks_ctas_per_sm;         /* > 0: cap of the peak scan's resident CTAs per SM */
-    int32_t reserved[9];               /* must be zero */
+    int32_t fill_store_warps;          /* 1: one store warp queues every tile store; 2: one store warp per slab (0: chosen
+                                          from the hits per plane of the call) */
+    int32_t reserved[8];               /* must be zero */
 } ht_tuning;
 
 /* Sizes implied by a configuration: bytes of one event's matrix, and bytes of the context's device workspace

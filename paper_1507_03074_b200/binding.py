@@ -56,7 +56,7 @@ class ht_tuning(C.Structure):
     _fields_ = [("fill_batch_classification", C.c_int32), ("fill_slab_kb", C.c_int32),
                 ("fill_plain_stores", C.c_int32), ("cooperative_launch", C.c_int32),
                 ("host_copy_input", C.c_int32), ("peaks_unroll", C.c_int32), ("peaks_ctas_per_sm", C.c_int32),
-                ("reserved", C.c_int32 * 9)]
+                ("fill_store_warps", C.c_int32), ("reserved", C.c_int32 * 8)]
 
 
 class HtError(RuntimeError):

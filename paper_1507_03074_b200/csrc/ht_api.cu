@@ -177,6 +177,7 @@ struct ht_ctx {
     ht_config cfg;
     ht_tuning tun;
     ht::Geom geom;
+    float two_a_absmax = 0.0f;             // max |2 * A_c| over the A rows
     int sm_count = 0;
     int max_smem_optin = 0;
     // device workspace
@@ -285,7 +286,7 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
         for (int32_t r : tun.reserved)
             if (r != 0) return HT_ERR_INVALID_ARG;
         if (tun.peaks_unroll != 0 && tun.peaks_unroll != 2 && tun.peaks_unroll != 4 && tun.peaks_unroll != 8) return HT_ERR_INVALID_ARG;
-        if (tun.fill_slab_kb < 0 || tun.peaks_ctas_per_sm < 0) return HT_ERR_INVALID_ARG;
+        if (tun.fill_slab_kb < 0 || tun.peaks_ctas_per_sm < 0 || tun.fill_store_warps < 0 || tun.fill_store_warps > 2) return HT_ERR_INVALID_ARG;
     }
     const WorkspaceLayout lay = workspace_layout(cfg);
     if (d_workspace && (workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0)) return HT_ERR_INVALID_ARG;
@@ -310,6 +311,11 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
     float d_ab[2];
     build_tables(cfg, nullptr, tth.data(), pph.data(), d_ab);
     g.a_min = cfg->a_min; g.dA = d_ab[0]; g.b_min = cfg->b_min; g.dB = d_ab[1]; g.nb_f = (float)cfg->n_b;
+    {   // 2 * A_c is monotone in the row: the largest magnitude is at one of the ends
+        std::vector<float> two_a((size_t)cfg->n_a);
+        build_tables(cfg, two_a.data(), tth.data(), pph.data(), d_ab);
+        ctx->two_a_absmax = std::max(std::fabs(two_a.front()), std::fabs(two_a.back()));
+    }
 
     cudaError_t e;
     auto fail = [&](int code) { ht_destroy(ctx); return code; };
@@ -492,6 +498,11 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.counts = ctx->d_counts; a.bucket_start = ctx->d_bucket_start; a.h_plane = ctx->d_hplane; a.h_rel = ctx->d_hrel;
     a.bx = pl.mode == 1 ? ctx->d_buckets : ctx->d_bx;
     a.bucket_cap = (int)align_up((size_t)n_hits_total, 4);
+    a.two_a_absmax = ctx->two_a_absmax;
+    // one queue of tile stores while the store is the slow part; a store warp per slab when the votes are (more than
+    // ~150 hits per (event, plane): config 4)
+    a.store_warps = ctx->tun.fill_store_warps ? ctx->tun.fill_store_warps
+                    : ((long long)n_hits_total > 150ll * (long long)n_events * (long long)g.planes ? 2 : 1);
     a.bar = ctx->d_counters + 2;
     a.g = g;
     a.rows_slab = pl.rows_slab;
@@ -920,7 +931,7 @@ int ht_diag_vote_rates(int32_t device, int32_t iters, double *h_rates, uint64_t 
     return HT_OK;
 }
 
-#ifdef HT_PROFILE_PHASES
+#ifdef HT_PROFILE_TIMELINE
 // build-time instrumentation only: copy (and clear) the per-CTA phase counters of the fill kernel
 __attribute__((visibility("default"))) int ht_prof_read(uint64_t *h_out, int32_t n_words, int32_t reset)
 {

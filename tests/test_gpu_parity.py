@@ -467,6 +467,8 @@ def test_error_codes_on_device_calls():
                                     {"fill_plain_stores": 1},            # plain stores instead of the TMA
                                     {"fill_batch_classification": 1, "fill_slab_kb": 8},
                                     {"cooperative_launch": 1},           # cudaLaunchCooperativeKernel instead of the dependent launch
+                                    {"fill_store_warps": 1}, {"fill_store_warps": 2},      # one queue of tile stores / a store warp per slab
+                                    {"fill_store_warps": 2, "fill_slab_kb": 8, "fill_batch_classification": 1},
                                     {"peaks_unroll": 4}, {"peaks_unroll": 8, "peaks_ctas_per_sm": 2}])
 def test_fill_kernel_variants_are_bit_exact(tuning):
     """The switches of ht_tuning (read once by ht_create_ex) change how the work is organised, never the result."""
