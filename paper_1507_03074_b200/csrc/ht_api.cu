@@ -117,12 +117,13 @@ void build_tables(const ht_config *c, float *two_a, float *tth, float *pph, floa
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 constexpr size_t kBucketBytesMax = 32u << 20;   // cap of the single-event bucket region (bigger events take the batch path)
+constexpr size_t kZeroBytes = 232448;           // 227 KB: no slab is larger
 constexpr size_t kResHeader = 16;      // result block: [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
 
 // Layout of the context's device workspace (one contiguous block: caller-owned or allocated by ht_create) and sizes of
 // the pinned host staging blocks.  Offsets are multiples of 256.
 struct WorkspaceLayout {
-    size_t tables, counters, hits, buckets, bucket_start, counts, in_dev, mh;      // offsets
+    size_t tables, counters, hits, buckets, bucket_start, counts, counts1, zeros, in_dev, mh;      // offsets
     size_t hits_part;             // bytes of one of the 6 per-hit arrays
     size_t buckets_bytes;         // single-event classification: P buckets of n_hits records each (as far as this holds them)
     size_t in_block, res_block;   // bytes of ONE slot's input block [offsets | x | y | z] and result block
@@ -144,6 +145,8 @@ WorkspaceLayout workspace_layout(const ht_config *c)
     w.buckets = take(w.buckets_bytes);
     w.bucket_start = take(sizeof(int32_t) * (size_t)c->max_events * (planes_all + 1));
     w.counts = take(sizeof(uint32_t) * (size_t)c->max_events * planes_all);
+    w.counts1 = take(sizeof(uint32_t) * planes_all * (size_t)ht::kCountStride);
+    w.zeros = take(kZeroBytes);                // source of the TMA's zero fill of a slab (at most the CTA's shared memory)
     if (c->host_slots > 0) {
         w.in_block = align_up(align_up(sizeof(int32_t) * ((size_t)c->max_events + 1), 16) +
                               3 * align_up(sizeof(float) * (size_t)c->max_hits, 16), 256);
@@ -192,6 +195,8 @@ struct ht_ctx {
     int32_t *d_hplane = nullptr, *d_hrel = nullptr;   // [max_hits] phase-1 spill
     int32_t *d_bucket_start = nullptr;     // [max_events * (P+1)]
     uint32_t *d_counts = nullptr;          // [max_events * P], zero between calls
+    uint32_t *d_counts1 = nullptr;         // [P * kCountStride], zero between calls
+    uint32_t *d_zeros = nullptr;           // kZeroBytes of zeros
     bool fill_ok = false;
     size_t fill_smem_max[2] = {0, 0};      // dynamic shared memory budget: [0] ht_fill, [1] fused peaks
     FillPlan plan_cache[2];
@@ -342,10 +347,14 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
     ctx->d_hrel = reinterpret_cast<int32_t *>(ws + lay.hits + 5 * lay.hits_part);
     ctx->d_bucket_start = reinterpret_cast<int32_t *>(ws + lay.bucket_start);
     ctx->d_counts = reinterpret_cast<uint32_t *>(ws + lay.counts);
+    ctx->d_counts1 = reinterpret_cast<uint32_t *>(ws + lay.counts1);
+    ctx->d_zeros = reinterpret_cast<uint32_t *>(ws + lay.zeros);
     if ((e = cudaMemset(ctx->d_counts, 0, align_up(sizeof(uint32_t) * (size_t)cfg->max_events * (size_t)(cfg->n_theta * cfg->n_phi), 256))) != cudaSuccess ||
         (e = cudaMemcpy(ctx->d_tth, tth.data(), tth.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMemcpy(ctx->d_pph, pph.data(), pph.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess ||
-        (e = cudaMemset(ctx->d_counters, 0, 256)) != cudaSuccess)
+        (e = cudaMemset(ctx->d_counters, 0, 256)) != cudaSuccess ||
+        (e = cudaMemset(ctx->d_zeros, 0, kZeroBytes)) != cudaSuccess ||
+        (e = cudaMemset(ctx->d_counts1, 0, sizeof(uint32_t) * (size_t)(cfg->n_theta * cfg->n_phi) * (size_t)ht::kCountStride)) != cudaSuccess)
         return fail(cuda_fail(e, "workspace initialisation"));
     if ((e = cudaEventCreateWithFlags(&ctx->order_event, cudaEventDisableTiming)) != cudaSuccess)
         return fail(cuda_fail(e, "cudaEventCreate"));
@@ -495,13 +504,14 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.x = d_x; a.y = d_y; a.z = d_z; a.event_offsets = d_off; a.n_events = n_events; a.n_hits = n_hits_total;
     a.tth = ctx->d_tth; a.pph = ctx->d_pph;
     a.mode = pl.mode;
-    a.counts = ctx->d_counts; a.bucket_start = ctx->d_bucket_start; a.h_plane = ctx->d_hplane; a.h_rel = ctx->d_hrel;
+    a.counts = ctx->d_counts; a.counts1 = ctx->d_counts1; a.zeros = ctx->d_zeros; a.bucket_start = ctx->d_bucket_start; a.h_plane = ctx->d_hplane; a.h_rel = ctx->d_hrel;
     a.bx = pl.mode == 1 ? ctx->d_buckets : ctx->d_bx;
     a.bucket_cap = (int)align_up((size_t)n_hits_total, 4);
     a.two_a_absmax = ctx->two_a_absmax;
     // one queue of tile stores while the store is the slow part; a store warp per slab when the votes are (more than
     // ~150 hits per (event, plane): config 4)
-    a.store_warps = ctx->tun.fill_store_warps ? ctx->tun.fill_store_warps
+    // (peaks only, no store: always one per slab -- the single queue exists for the stores' sake)
+    a.store_warps = !d_mh ? 2 : ctx->tun.fill_store_warps ? ctx->tun.fill_store_warps
                     : ((long long)n_hits_total > 150ll * (long long)n_events * (long long)g.planes ? 2 : 1);
     a.bar = ctx->d_counters + 2;
     a.g = g;

@@ -64,7 +64,7 @@ def test_tables_bit_identical_to_the_oracle(bn):
 def test_query_sizes_and_argument_validation():
     cfg = B.ht_config.from_binning(WORKLOADS[2].binning, max_events=2, max_hits=5000)
     mh, ws = B.ht_query_sizes(cfg)
-    assert mh == 4 * 67_108_864 and 0 < ws < (1 << 23) and ws % 256 == 0     # incl. 64 plane buckets x 5000 records
+    assert mh == 4 * 67_108_864 and 0 < ws < (1 << 24) and ws % 256 == 0     # incl. 64 plane buckets x 5000 records
     cfg_h = B.ht_config.from_binning(WORKLOADS[1].binning, max_events=2, max_hits=100, host_slots=2, host_peak_capacity=100)
     mh1, ws1 = B.ht_query_sizes(cfg_h)
     assert ws1 > 2 * mh1
