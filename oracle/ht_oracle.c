@@ -24,10 +24,13 @@
  * mirror symmetry (P6), permutation/batching invariance (P7), hand-built peak matrices (P8),
  * peak-set invariants (P9), table binning vs atan2 (P10), closed-form in-range fraction; track read-out: the
  * truth circle of a noiseless track (P11), polar identities and special cells (P12); ridge merging: connected-component
- * labelling of a library routine on a doubled grid (P13), hand-built peak layouts (P14), partition invariants (P15).
+ * labelling of a library routine on a doubled grid (P13), hand-built peak layouts (P14), partition invariants (P15); truth
+ * matching: noiseless tracks through generator, fill, peaks and merge (P16), a sector-split soft track (P17), hand-built
+ * lists (P18), invariants and a brute force in polar coordinates (P19).
  * Parity unpinned by the paper (definitions fixed by SPEC.md only): R2/R4 angle definition and
  * ranges, R5 bin centre, R10 neighbourhood, R11 >= vs >, R12 tie rule, R17 quadrant of phi, R19 (the merge rule itself
- * is this build's stand-in for the paper's unexplained step from local maxima to tracks).
+ * is this build's stand-in for the paper's unexplained step from local maxima to tracks), R20 (the matching rule: the
+ * paper's own comparison is against a chi^2 fit on its dataset, both unavailable).
  */
 #include <math.h>
 #include <stdint.h>

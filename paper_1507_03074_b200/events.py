@@ -190,6 +190,45 @@ def generate_batch(workload: Workload | int, *, n_events: int | None = None, see
                       event_offsets=np.asarray(offs, dtype=np.int32), truth=truths)
 
 
+def truth_table(batch: EventBatch, n_theta: int | None = None, n_phi: int | None = None) -> dict:
+    """Generator truth of a batch as flat arrays, one entry per generated track (geometry of the generator only, G2/G3):
+    ``event``; centre ``a, b`` of the track's circle through the origin, ``R * (q sin phi0, -q cos phi0)`` (mm, float64);
+    its radius ``rho`` and the azimuth ``phi`` of the centre in (-pi, pi]; ``n_hits`` of the track that are in the event
+    (12, fewer for the truncated last track of a fixed-total event); and, if a segmentation is given, ``max_sector_hits``:
+    the largest number of the track's (unsmeared) hits inside ONE of the n_theta x n_phi equal sectors in polar angle
+    and azimuth -- a soft track curls across azimuthal sectors, so not all of its 12 hits share one."""
+    ev, a, b, rho, nh, msh = [], [], [], [], [], []
+    r = layer_radii()[None, :]
+    for e, tr in enumerate(batch.truth):
+        q, radius, phi0, eta = tr["q"], tr["radius"], tr["phi0"], tr["eta"]
+        n_tr = q.shape[0]
+        kept = np.clip(tr["n_track_hits"] - N_LAYERS * np.arange(n_tr), 0, N_LAYERS)     # hits are track-major, layer-minor
+        ev.append(np.full(n_tr, e, np.uint32))
+        a.append(radius * q * np.sin(phi0))
+        b.append(-radius * q * np.cos(phi0))
+        rho.append(radius)
+        nh.append(kept)
+        if n_theta and n_phi:
+            psi = 2.0 * np.arcsin(r / (2.0 * radius[:, None]))
+            phi_hit = np.mod(phi0[:, None] - q[:, None] * psi / 2.0, 2.0 * math.pi)
+            theta_hit = np.arctan2(r, radius[:, None] * psi * np.sinh(eta)[:, None])        # polar angle from the +z axis, (0, pi)
+            sec = (np.minimum((theta_hit / (math.pi / n_theta)).astype(np.int64), n_theta - 1) * n_phi
+                   + np.minimum((phi_hit / (2.0 * math.pi / n_phi)).astype(np.int64), n_phi - 1))
+            have = np.arange(N_LAYERS)[None, :] < kept[:, None]
+            m = np.zeros(n_tr, np.int64)
+            for k in range(n_tr):
+                if kept[k]:
+                    m[k] = np.bincount(sec[k][have[k]]).max()
+            msh.append(m)
+    cat = lambda parts, dt: np.concatenate(parts).astype(dt) if parts else np.zeros(0, dt)
+    out = dict(event=cat(ev, np.uint32), a=cat(a, np.float64), b=cat(b, np.float64), rho=cat(rho, np.float64),
+               n_hits=cat(nh, np.int64))
+    out["phi"] = np.arctan2(out["b"], out["a"])
+    if n_theta and n_phi:
+        out["max_sector_hits"] = cat(msh, np.int64)
+    return out
+
+
 def batch_from_arrays(events: list[np.ndarray]) -> EventBatch:
     """Pack hand-built events ([n_i,3] arrays) into an EventBatch (used by tests for edge cases)."""
     offs = [0]

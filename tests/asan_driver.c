@@ -45,14 +45,24 @@ int main(int argc, char **argv)
     oracle_tracks(&g, pk, np, rho, phi);
     oracle_merged *mg = (oracle_merged *)malloc(sizeof(oracle_merged) * (size_t)(np + 1));
     const int64_t nm = oracle_merge_ridges(&g, pk, np, window, mg, np);
+    /* truth matching of the candidates against a few circles derived from the hits themselves (any input will do here:
+       the point is that every access of oracle_match_truth runs under the sanitizers) */
+    const int64_t nt = n < 64 ? n : 64;
+    oracle_truth *tr = (oracle_truth *)malloc(sizeof(oracle_truth) * (size_t)(nt + 1));
+    for (int64_t k = 0; k < nt; ++k) { tr[k].event = (uint32_t)(k & 1); tr[k].pad = 0u; tr[k].a = 3.0 * x[k]; tr[k].b = -2.5 * y[k]; }
+    int32_t *cmatch = (int32_t *)malloc(4 * (size_t)(nm + 1)), *tmatch = (int32_t *)malloc(4 * (size_t)(nt + 1));
+    oracle_match_summary ms;
+    const int mrc = oracle_match_truth(&g, mg, nm > 0 ? nm : 0, tr, nt, 200.0, 0.95, cmatch, tmatch, &ms);
     uint64_t h = 1469598103934665603ull;
     h = fnv(M, cells * 4, h);
+    printf("match_rc %d found %lld fake %lld match_hash %llu ", mrc, (long long)ms.n_found, (long long)ms.n_fake,
+           (unsigned long long)fnv(cmatch, 4 * (size_t)(nm > 0 ? nm : 0), fnv(tmatch, 4 * (size_t)nt, 7)));
     printf("votes %lld matrix_hash %llu peaks %lld peaks_hash %llu tracks_hash %llu merged %lld merged_hash %llu planes_hash %llu\n",
            (long long)votes, (unsigned long long)h, (long long)np,
            (unsigned long long)fnv(pk, sizeof(oracle_peak) * (size_t)np, 7),
            (unsigned long long)fnv(rho, 8 * (size_t)np, fnv(phi, 8 * (size_t)np, 7)), (long long)nm,
            (unsigned long long)fnv(mg, sizeof(oracle_merged) * (size_t)(nm > 0 ? nm : 0), 7),
            (unsigned long long)fnv(plane, 4 * (size_t)n, fnv(bins, 4 * (size_t)n * (size_t)g.n_a, 7)));
-    free(x); free(y); free(z); free(M); free(plane); free(bins); free(pk); free(rho); free(phi); free(mg);
+    free(x); free(y); free(z); free(M); free(plane); free(bins); free(pk); free(rho); free(phi); free(mg); free(tr); free(cmatch); free(tmatch);
     return 0;
 }

@@ -1,0 +1,203 @@
+"""Pins of oracle_match_truth (SPEC.md section 6, reading R20) -- none re-types its arithmetic:
+
+P16  geometry the paper fixes (PAPER.md:25 circles through the interaction point; PAPER.md:29 rho, phi of the centre):
+     noiseless, well separated tracks whose 12 hits share one (theta, phi) sector, through generator geometry -> fill ->
+     peaks -> ridge merging -> matching: every track found, no fake, residuals below one cell diagonal;
+P17  the negative case of reading R2: a soft track whose hits split 7 + 5 over two azimuthal sectors makes no peak at
+     threshold 8, so it is not found (and nothing fake appears);
+P18  hand-built candidate and truth lists with hand-computed outcomes (exact matches, a radial and an azimuthal miss,
+     window edges, duplicates, other events);
+P19  invariants on random lists, and agreement with a brute force written in polar coordinates (angle differences by
+     arctangent instead of the oracle's dot-product test) away from the window edges.
+"""
+import math
+
+import numpy as np
+
+from oracle import (MERGED_DTYPE, TRUTH_DTYPE, oracle_fill, oracle_match_truth, oracle_merge_ridges, oracle_peaks,
+                    oracle_tracks, PEAK_DTYPE)
+from paper_1507_03074_b200.events import Binning, layer_radii
+
+
+def _circle_hits(radius, q, phi0, z_slope):
+    r = layer_radii()
+    psi = 2.0 * np.arcsin(r / (2.0 * radius))
+    ph = phi0 - q * psi / 2.0
+    return np.stack([r * np.cos(ph), r * np.sin(ph), z_slope * r], axis=-1).astype(np.float32)
+
+
+def _truth(recs):
+    t = np.zeros(len(recs), TRUTH_DTYPE)
+    for i, (e, a, b) in enumerate(recs):
+        t[i] = (e, 0, a, b)
+    return t
+
+
+def _cands(bn, recs):
+    """MERGED_DTYPE records for (event, ia, ib) cells of plane 0 (rho, phi filled in by the oracle's own read-out)."""
+    c = np.zeros(len(recs), MERGED_DTYPE)
+    pk = np.zeros(len(recs), PEAK_DTYPE)
+    for i, (e, ia, ib) in enumerate(recs):
+        pk[i] = (e, ia * bn.n_b + ib, 12)
+    rho, phi = oracle_tracks(bn, pk)
+    c["event"], c["cell"], c["count"], c["n_peaks"], c["rho"], c["phi"] = pk["event"], pk["cell"], 12, 1, rho, phi
+    return c
+
+
+def _centred_track(radius, q, sector, z_slope, n_phi=16):
+    """(R, q, phi0, z/r) of a track whose 12 hit azimuths are centred in azimuthal sector `sector`."""
+    swing_out, swing_in = math.asin(1000.0 / (2 * radius)), math.asin(50.0 / (2 * radius))
+    return radius, q, (sector + 0.5) * (2 * math.pi / n_phi) + q * (swing_out + swing_in) / 2, z_slope
+
+
+def test_p16_noiseless_separated_tracks_are_all_found_with_ridge_sized_residuals():
+    bn = Binning(4, 16, 1024, 1024)
+    d = 8000.0 / 1024
+    diag = math.hypot(d, d)
+    # Eight tracks, far apart, each with its 12 hits inside one 22.5 degree sector and one theta bin, in the sectors where
+    # |x/y| <= 1 (nearer the x axis a vote line advances several B bins per A row and, with one vote per row -- R7 -- the
+    # twelve lines no longer meet in one cell: a property of the method as specified, not of this test).
+    tracks = [_centred_track(1500.0, +1.0, 2, 0.3), _centred_track(1700.0, -1.0, 3, 0.5), _centred_track(2200.0, +1.0, 4, 0.2),
+              _centred_track(2600.0, -1.0, 5, 0.4), _centred_track(1600.0, -1.0, 10, 0.6), _centred_track(3000.0, +1.0, 11, 0.25),
+              _centred_track(3300.0, -1.0, 12, 0.3), _centred_track(1900.0, +1.0, 13, 0.45)]
+    hits, truth = [], []
+    for radius, q, phi0, zs in tracks:
+        hits.append(_circle_hits(radius, q, phi0, zs))
+        truth.append((0, radius * q * math.sin(phi0), -radius * q * math.cos(phi0)))      # generator G3
+    xyz = np.concatenate(hits)
+    m, _ = oracle_fill(bn, xyz[:, 0], xyz[:, 1], xyz[:, 2])
+    assert m.max() == 12
+    peaks = oracle_peaks(bn, m, 8)
+    assert len(peaks) > 8                                           # ridges: several local maxima per track ...
+    cands = oracle_merge_ridges(bn, peaks, 10)
+    assert len(cands) == 8 and np.all(cands["count"] == 12)         # ... one candidate per track after merging
+    tr = _truth(truth)
+    cm, tm, s = oracle_match_truth(bn, cands, tr, w_rho=6 * d, cos_w_phi=math.cos(0.03))
+    assert s["n_truth"] == 8 and s["n_found"] == 8, s               # efficiency 1
+    assert s["n_fake"] == 0 and s["n_duplicate"] == 0               # fake rate 0
+    assert sorted(tm.tolist()) == list(range(8)) and sorted(cm.tolist()) == list(range(8))
+    for t in range(8):
+        c = cands[tm[t]]
+        radius = tracks[t][0]
+        want = math.atan2(truth[t][2], truth[t][1])
+        dphi = (c["phi"] - want + math.pi) % (2 * math.pi) - math.pi
+        # the twelve lines of a stiff track are nearly parallel: the maximum is a ridge a few cells long, and the
+        # representative is one of its 12-vote cells; a curlier track pins its centre down to about a cell
+        bound = (2 if radius <= 2000.0 else 5) * diag
+        assert abs(c["rho"] - radius) <= bound and radius * abs(dphi) <= bound, (t, c["rho"] - radius, radius * dphi)
+    assert math.sqrt(s["sum_drho2"] / 8) <= 3 * diag
+
+
+def test_p17_a_soft_track_split_by_a_sector_edge_is_not_found():
+    bn = Binning(4, 16, 1024, 1024)
+    # R = 930 mm: the hit azimuth swings by 32 degrees over the layers; started so that 7 hits fall into one phi sector
+    # and 5 into the next (SURVEY.md 8(c), P2's negative case)
+    radius, q, zs = 930.0, 1.0, 0.3
+    edge = 2 * math.pi / 16 * 3
+    r = layer_radii()
+    swing = np.arcsin(r / (2.0 * radius))
+    phi0 = edge + 0.5 * (swing[6] + swing[7])                       # hits 0..6 above the edge, 7..11 below
+    xyz = _circle_hits(radius, q, phi0, zs)
+    az = np.mod(np.arctan2(xyz[:, 1].astype(np.float64), xyz[:, 0].astype(np.float64)), 2 * math.pi)
+    assert sorted(np.bincount((az / (2 * math.pi / 16)).astype(int), minlength=16)[[2, 3]].tolist()) == [5, 7]
+    m, _ = oracle_fill(bn, xyz[:, 0], xyz[:, 1], xyz[:, 2])
+    assert m.max() == 7
+    cands = oracle_merge_ridges(bn, oracle_peaks(bn, m, 8), 3)
+    tr = _truth([(0, radius * q * math.sin(phi0), -radius * q * math.cos(phi0))])
+    cm, tm, s = oracle_match_truth(bn, cands, tr, w_rho=40.0, cos_w_phi=math.cos(0.05))
+    assert len(cands) == 0 and s["n_found"] == 0 and tm[0] == -1 and s["n_fake"] == 0
+    # at threshold 7 the larger half peaks, and that peak IS the track (same circle centre)
+    cands7 = oracle_merge_ridges(bn, oracle_peaks(bn, m, 7), 3)
+    _, tm7, s7 = oracle_match_truth(bn, cands7, tr, w_rho=40.0, cos_w_phi=math.cos(0.05))
+    assert s7["n_found"] == 1 and tm7[0] >= 0
+
+
+def test_p18_hand_built_lists():
+    bn = Binning(1, 1, 100, 100, a_min=-500.0, a_max=500.0, b_min=-500.0, b_max=500.0)   # 10 mm cells, centres -495 .. 495
+    # candidates (event, ia, ib) -> centres: (305, 5), (315, 5), (5, 305), (-295, 5), (305, 5) in event 1
+    cands = _cands(bn, [(0, 80, 50), (0, 81, 50), (0, 50, 80), (0, 20, 50), (1, 80, 50)])
+    truth = _truth([(0, 304.0, 5.0),        # t0: 1 mm from candidate 0, 11 mm from candidate 1
+                    (0, 5.0, 330.0),        # t1: 25 mm radially from candidate 2
+                    (0, -295.0, 40.0),      # t2: same radius as candidate 3 within 3 mm, 35 mm away tangentially (0.118 rad)
+                    (2, 305.0, 5.0)])       # t3: event 2 has no candidate
+    # windows: 12 mm in rho, 0.05 rad in phi
+    cm, tm, s = oracle_match_truth(bn, cands, truth, 12.0, math.cos(0.05))
+    assert cm.tolist() == [0, 0, -1, -1, -1]        # c0, c1 -> t0; c2 radial miss; c3 azimuthal miss; c4 other event
+    assert tm.tolist() == [0, -1, -1, -1]           # t0's best candidate is c0 (1 mm against 11 mm)
+    assert (s["n_cand"], s["n_truth"], s["n_matched"], s["n_fake"], s["n_found"], s["n_duplicate"]) == (5, 4, 2, 3, 1, 1)
+    assert abs(s["sum_drho"] - (math.hypot(305.0, 5.0) - math.hypot(304.0, 5.0))) < 1e-9
+    assert abs(s["sum_dphi"] - (math.atan2(5.0, 305.0) - math.atan2(5.0, 304.0))) < 1e-12
+    # wider windows: 30 mm and 0.2 rad pick up c2 -> t1 and c3 -> t2
+    cm, tm, s = oracle_match_truth(bn, cands, truth, 30.0, math.cos(0.2))
+    assert cm.tolist() == [0, 0, 1, 2, -1] and tm.tolist() == [0, 2, 3, -1]
+    assert (s["n_matched"], s["n_fake"], s["n_found"], s["n_duplicate"]) == (4, 1, 3, 1)
+    # the window edges are inclusive: a candidate exactly w_rho away (same direction) matches, a hair less does not
+    c1 = _cands(bn, [(0, 80, 50)])
+    sc = 1.0 + 12.0 / math.hypot(305.0, 5.0)
+    t_edge = _truth([(0, 305.0 * sc, 5.0 * sc)])
+    rho_c, rho_t = math.sqrt(305.0 * 305.0 + 5.0 * 5.0), math.sqrt((305.0 * sc) ** 2 + (5.0 * sc) ** 2)
+    gap = abs(rho_c - rho_t)
+    assert oracle_match_truth(bn, c1, t_edge, gap, 0.999)[0].tolist() == [0]
+    assert oracle_match_truth(bn, c1, t_edge, math.nextafter(gap, 0.0), 0.999)[0].tolist() == [-1]
+    # empty lists
+    cm, tm, s = oracle_match_truth(bn, cands[:0], truth, 12.0, 0.99)
+    assert len(cm) == 0 and tm.tolist() == [-1] * 4 and s["n_found"] == 0
+    cm, tm, s = oracle_match_truth(bn, cands, truth[:0], 12.0, 0.99)
+    assert cm.tolist() == [-1] * 5 and s["n_fake"] == 5
+
+
+def test_p19_invariants_and_polar_brute_force():
+    bn = Binning(2, 4, 256, 256)
+    dA = 8000.0 / 256
+    rng = np.random.default_rng(19)
+    for trial in range(8):
+        n_t, n_c = int(rng.integers(5, 60)), int(rng.integers(5, 120))
+        tr = np.zeros(n_t, TRUTH_DTYPE)
+        tr["event"] = rng.integers(0, 3, n_t)
+        ang, rad = rng.uniform(-math.pi, math.pi, n_t), rng.uniform(900.0, 3800.0, n_t)
+        tr["a"], tr["b"] = rad * np.cos(ang), rad * np.sin(ang)
+        recs = []
+        for k in range(n_c):                                        # half of the candidates near a truth centre, half anywhere
+            if k % 2 == 0:
+                t = int(rng.integers(0, n_t))
+                ia = int(np.clip((tr["a"][t] + 4000.0) / dA + rng.integers(-3, 4), 0, 255))
+                ib = int(np.clip((tr["b"][t] + 4000.0) / dA + rng.integers(-3, 4), 0, 255))
+                recs.append((int(tr["event"][t]), ia, ib))
+            else:
+                recs.append((int(rng.integers(0, 3)), int(rng.integers(0, 256)), int(rng.integers(0, 256))))
+        recs = sorted(set(recs))
+        cd = _cands(bn, recs)
+        w_rho, w_phi = 2.5 * dA, 0.03
+        cm, tm, s = oracle_match_truth(bn, cd, tr, w_rho, math.cos(w_phi))
+        # invariants
+        assert s["n_matched"] + s["n_fake"] == len(cd) and s["n_found"] + s["n_duplicate"] == s["n_matched"]
+        assert s["n_found"] == int((tm >= 0).sum()) <= min(n_t, len(cd))
+        assert all(cm[tm[t]] == t for t in range(n_t) if tm[t] >= 0)
+        # permutation of both lists: the same pairs, keyed by (event, cell) and by the truth record
+        pc, pt = rng.permutation(len(cd)), rng.permutation(n_t)
+        cm2, tm2, s2 = oracle_match_truth(bn, cd[pc], tr[pt], w_rho, math.cos(w_phi))
+        assert {k: s2[k] for k in s if k.startswith("n_")} == {k: s[k] for k in s if k.startswith("n_")}
+        assert [(-1 if c < 0 else int(pt[c])) for c in cm2] == cm[pc].tolist()
+        assert [(-1 if c < 0 else int(pc[c])) for c in tm2] == tm[pt].tolist()
+        # wider windows never lose a match
+        cm3, _, s3 = oracle_match_truth(bn, cd, tr, 2 * w_rho, math.cos(2 * w_phi))
+        assert np.all((cm3 >= 0) | (cm < 0)) and s3["n_found"] >= s["n_found"]
+        # brute force in polar coordinates, away from the window edges
+        ac = -4000.0 + (np.array([r[1] for r in recs]) + 0.5) * dA
+        bc = -4000.0 + (np.array([r[2] for r in recs]) + 0.5) * dA
+        for c in range(len(cd)):
+            best, best_d = -1, None
+            sure = True
+            for t in range(n_t):
+                if tr["event"][t] != cd["event"][c]:
+                    continue
+                drho = abs(math.hypot(ac[c], bc[c]) - math.hypot(tr["a"][t], tr["b"][t]))
+                dphi = abs((math.atan2(bc[c], ac[c]) - math.atan2(tr["b"][t], tr["a"][t]) + math.pi) % (2 * math.pi) - math.pi)
+                if abs(drho - w_rho) < 1e-6 or abs(dphi - w_phi) < 1e-9:
+                    sure = False
+                if drho <= w_rho and dphi <= w_phi:
+                    d2 = (ac[c] - tr["a"][t]) ** 2 + (bc[c] - tr["b"][t]) ** 2
+                    if best < 0 or d2 < best_d:
+                        best, best_d = t, d2
+            if sure:
+                assert cm[c] == best

@@ -8,7 +8,7 @@ import subprocess
 
 import numpy as np
 
-from oracle import oracle_fill, oracle_merge_ridges, oracle_peaks, oracle_tracks, oracle_votes
+from oracle import TRUTH_DTYPE, oracle_fill, oracle_match_truth, oracle_merge_ridges, oracle_peaks, oracle_tracks, oracle_votes
 from paper_1507_03074_b200.events import WORKLOADS, generate_batch
 
 HERE = os.path.dirname(os.path.abspath(__file__))
@@ -56,3 +56,10 @@ def test_oracle_is_clean_under_asan_and_ubsan(tmp_path):
     assert got["tracks_hash"] == _fnv(rho.tobytes(), _fnv(phi.tobytes(), 7))
     assert got["merged_hash"] == _fnv(mg.tobytes(), 7)
     assert got["planes_hash"] == _fnv(plane.tobytes(), _fnv(bins.tobytes(), 7))
+    nt = min(len(x), 64)
+    tr = np.zeros(nt, TRUTH_DTYPE)
+    tr["event"] = np.arange(nt) & 1
+    tr["a"], tr["b"] = 3.0 * x[:nt].astype(np.float64), -2.5 * y[:nt].astype(np.float64)
+    cm, tm, s = oracle_match_truth(bn, mg, tr, 200.0, 0.95)
+    assert got["match_rc"] == 0 and got["found"] == s["n_found"] and got["fake"] == s["n_fake"]
+    assert got["match_hash"] == _fnv(cm.tobytes(), _fnv(tm.tobytes(), 7))
