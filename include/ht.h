@@ -194,6 +194,53 @@ typedef struct ht_track {
  */
 HT_API int ht_tracks(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, ht_track *d_out, void *cuda_stream);
 
+/* A track candidate: a connected group of peaks of one ridge (f3; SPEC.md section 5, reading R19). */
+typedef struct ht_candidate {
+    uint32_t event, cell, count; /* the representative peak: largest count of the group, smallest cell among equals */
+    uint32_t n_peaks;            /* peaks merged into this candidate */
+    float rho, phi;              /* read-out of the representative's cell, as ht_track */
+} ht_candidate;
+
+/*
+ * Ridge merging of a peak list into track candidates (PAPER.md:25 goes from "local maxima" straight to "real tracks";
+ * SURVEY.md section 8(f) f3 "merging ridge peaks"; SPEC.md section 5): peaks of the same event and (theta,phi) plane whose
+ * (a, b) cells are at Chebyshev distance <= window are linked; a candidate is a connected component of the link graph.
+ *   d_peaks    device, n_peaks records (any order); records with event >= cfg.max_events are ignored
+ *   d_out      device, room for `capacity` candidates, order unspecified (compare sorted by (event, cell))
+ *   d_n_out    device, one uint32: the number of candidates (may exceed capacity; then only `capacity` were written)
+ *   d_scratch  device, at least ht_merge_scratch_bytes(n_peaks) bytes, 4-byte aligned, caller-owned
+ * Enqueues a few small kernels on cuda_stream (they use the context's (event, plane) counters: stream-ordered with the
+ * other calls of the context like every enqueuing call).
+ */
+HT_API size_t ht_merge_scratch_bytes(uint32_t n_peaks);
+HT_API int ht_merge_ridges(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, uint32_t window, ht_candidate *d_out,
+                           uint32_t capacity, uint32_t *d_n_out, void *d_scratch, size_t scratch_bytes, void *cuda_stream);
+
+/* A generated track for ht_match_truth: the centre (a, b) [mm] of its circle through the origin, R (q sin phi0, -q cos phi0). */
+typedef struct ht_truth {
+    uint32_t event, pad;
+    double a, b;
+} ht_truth;
+
+typedef struct ht_match_summary {
+    int64_t n_cand, n_truth, n_matched, n_fake, n_found, n_duplicate;
+    double sum_drho, sum_drho2, sum_dphi, sum_dphi2; /* residuals rho_c - rho_t [mm] and phi_c - phi_t [rad] of the found tracks */
+} ht_match_summary;
+
+/*
+ * Truth matching of track candidates (stand-in for PAPER.md:29-33, Fig. 1: the tracks' rho, phi "together with the
+ * corresponding resolutions"; SURVEY.md section 8(f) f3 "truth-matched efficiency / fake rate / resolution"; SPEC.md
+ * section 6, reading R20).  Candidate c and truth t are compatible when they belong to the same event,
+ * |rho_c - rho_t| <= w_rho and the angle between their centres is <= w_phi (cos_w_phi = cos(w_phi), taken by the caller).
+ *   d_cand_match   device, n_cand int32: the closest compatible truth record, or -1 (the candidate is a fake)
+ *   d_truth_match  device, n_truth int32: the closest candidate matched to it, or -1 (not found)
+ *   d_summary      device, one ht_match_summary (efficiency = n_found / n_truth, fake rate = n_fake / n_cand)
+ * All decisions in binary64; O(n_cand * n_truth) work, meant for evaluation, not for the hot path.
+ */
+HT_API int ht_match_truth(ht_ctx *ctx, const ht_candidate *d_cand, uint32_t n_cand, const ht_truth *d_truth, uint32_t n_truth,
+                          double w_rho, double cos_w_phi, int32_t *d_cand_match, int32_t *d_truth_match,
+                          ht_match_summary *d_summary, void *cuda_stream);
+
 /*
  * End-to-end call with HOST buffers (f4; needs cfg.host_slots >= 1; the transfer is "the dominant part" of
  * the paper's total time -- here only the hits (12 bytes each) and the compacted peak list cross PCIe).

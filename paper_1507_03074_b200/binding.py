@@ -21,7 +21,15 @@ PEAK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.u
 TRACK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32),
                         ("rho", np.float32), ("phi", np.float32)])                                # == struct ht_track
 
+CAND_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32), ("n_peaks", np.uint32),
+                       ("rho", np.float32), ("phi", np.float32)])                                 # == struct ht_candidate
+TRUTH_DTYPE = np.dtype([("event", np.uint32), ("pad", np.uint32), ("a", np.float64), ("b", np.float64)])   # == struct ht_truth
+SUMMARY_DTYPE = np.dtype([("n_cand", np.int64), ("n_truth", np.int64), ("n_matched", np.int64), ("n_fake", np.int64),
+                          ("n_found", np.int64), ("n_duplicate", np.int64), ("sum_drho", np.float64),
+                          ("sum_drho2", np.float64), ("sum_dphi", np.float64), ("sum_dphi2", np.float64)])   # == ht_match_summary
+
 EXPORTS = ("ht_query_sizes", "ht_create", "ht_create_ex", "ht_fill", "ht_fill_peaks", "ht_fill_naive", "ht_peaks", "ht_tracks",
+           "ht_merge_scratch_bytes", "ht_merge_ridges", "ht_match_truth",
            "ht_run_host", "ht_submit_host", "ht_wait_host", "ht_destroy", "ht_strerror")                  # include/ht.h
 DIAG_EXPORTS = ("ht_tables_host", "ht_kernel_launches", "ht_launch_info", "ht_selftest_division", "ht_diag_memset",
                 "ht_diag_vote_rates")                                                                     # include/ht_diag.h
@@ -105,6 +113,12 @@ def load() -> C.CDLL:
     lib.ht_peaks.argtypes = [vp, vp, i32, u32, vp, u32, vp, vp]
     lib.ht_tracks.restype = C.c_int
     lib.ht_tracks.argtypes = [vp, vp, u32, vp, vp]
+    lib.ht_merge_scratch_bytes.restype = C.c_size_t
+    lib.ht_merge_scratch_bytes.argtypes = [u32]
+    lib.ht_merge_ridges.restype = C.c_int
+    lib.ht_merge_ridges.argtypes = [vp, vp, u32, u32, vp, u32, vp, vp, C.c_size_t, vp]
+    lib.ht_match_truth.restype = C.c_int
+    lib.ht_match_truth.argtypes = [vp, vp, u32, vp, u32, C.c_double, C.c_double, vp, vp, vp, vp]
     lib.ht_run_host.restype = C.c_int
     lib.ht_run_host.argtypes = [vp, vp, vp, vp, vp, i32, i32, u32, vp, u32, vp, vp]
     lib.ht_selftest_division.restype = C.c_int
@@ -208,6 +222,24 @@ def ht_peaks(ctx, d_mh, n_events: int, threshold: int, d_out, capacity: int, d_n
 def ht_tracks(ctx, d_peaks, n_peaks: int, d_out, stream=None) -> None:
     """(rho, phi) of n_peaks peak records: d_out receives n_peaks ht_track records (5 words each)."""
     _check(load().ht_tracks(ctx, _ptr(d_peaks), n_peaks, _ptr(d_out), _stream(stream)), "ht_tracks")
+
+
+def ht_merge_scratch_bytes(n_peaks: int) -> int:
+    return int(load().ht_merge_scratch_bytes(n_peaks))
+
+
+def ht_merge_ridges(ctx, d_peaks, n_peaks: int, window: int, d_out, capacity: int, d_n_out, d_scratch, scratch_bytes: int,
+                    stream=None) -> None:
+    """Ridge merging of n_peaks peak records into track candidates (ht_candidate records, 6 words each)."""
+    _check(load().ht_merge_ridges(ctx, _ptr(d_peaks), n_peaks, window, _ptr(d_out), capacity, _ptr(d_n_out), _ptr(d_scratch),
+                                  scratch_bytes, _stream(stream)), "ht_merge_ridges")
+
+
+def ht_match_truth(ctx, d_cand, n_cand: int, d_truth, n_truth: int, w_rho: float, cos_w_phi: float, d_cand_match,
+                   d_truth_match, d_summary, stream=None) -> None:
+    """Truth matching of n_cand candidates against n_truth generated circles (ht_truth records)."""
+    _check(load().ht_match_truth(ctx, _ptr(d_cand), n_cand, _ptr(d_truth), n_truth, float(w_rho), float(cos_w_phi),
+                                 _ptr(d_cand_match), _ptr(d_truth_match), _ptr(d_summary), _stream(stream)), "ht_match_truth")
 
 
 def ht_run_host(ctx, h_x, h_y, h_z, h_event_offsets, n_events: int, n_hits_total: int, threshold: int, h_out,

@@ -5,6 +5,7 @@
 #include "../../include/ht_diag.h"
 #include "ht_device.cuh"
 #include "ht_diag.cuh"
+#include "ht_merge.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -859,6 +860,64 @@ int ht_tracks(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, ht_track *d
         reinterpret_cast<const ht::PeakOut *>(d_peaks), n_peaks, ctx->geom, reinterpret_cast<ht::TrackOut *>(d_out));
     HT_CUDA(cudaGetLastError());
     ++ctx->launches;
+    return HT_OK;
+}
+
+size_t ht_merge_scratch_bytes(uint32_t n_peaks) { return 3u * sizeof(uint32_t) * (size_t)(n_peaks ? n_peaks : 1u); }
+
+int ht_merge_ridges(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, uint32_t window, ht_candidate *d_out, uint32_t capacity,
+                    uint32_t *d_n_out, void *d_scratch, size_t scratch_bytes, void *cuda_stream)
+{
+    if (!ctx || !d_n_out || (capacity > 0 && !d_out)) return HT_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    HT_CUDA(cudaMemsetAsync(d_n_out, 0, sizeof(uint32_t), st));
+    if (n_peaks == 0u) return HT_OK;
+    if (!d_peaks || !d_scratch || scratch_bytes < ht_merge_scratch_bytes(n_peaks) ||
+        (reinterpret_cast<uintptr_t>(d_scratch) & 3u) != 0) return HT_ERR_INVALID_ARG;
+    static_assert(sizeof(ht::CandOut) == sizeof(ht_candidate), "candidate record layout");
+    const int ro = order_after_previous(ctx, st);
+    if (ro != HT_OK) return ro;
+    const int planes_all = ctx->cfg.n_theta * ctx->cfg.n_phi;
+    const unsigned long long groups = (unsigned long long)ctx->cfg.max_events * (unsigned long long)planes_all;
+    if (groups >= (1ull << 31)) return HT_ERR_UNSUPPORTED;
+    uint32_t *slot = static_cast<uint32_t *>(d_scratch), *order = slot + n_peaks, *label = order + n_peaks;
+    const ht::PeakOut *pk = reinterpret_cast<const ht::PeakOut *>(d_peaks);
+    const unsigned threads = 256, blocks = (n_peaks + threads - 1u) / threads;
+    ht::merge_count_kernel<<<blocks, threads, 0, st>>>(pk, n_peaks, ctx->geom, planes_all, (uint32_t)ctx->cfg.max_events,
+                                                       ctx->d_counts, slot);
+    ht::merge_scan_kernel<<<1, 1024, 0, st>>>(ctx->d_counts, ctx->d_bucket_start, (uint32_t)groups);
+    ht::merge_scatter_kernel<<<blocks, threads, 0, st>>>(pk, n_peaks, ctx->geom, planes_all, ctx->d_bucket_start, slot, order);
+    ht::merge_groups_kernel<<<(unsigned)groups, 128, 0, st>>>(pk, ctx->geom, ctx->d_bucket_start, order, label, window,
+                                                              reinterpret_cast<ht::CandOut *>(d_out), capacity, d_n_out);
+    HT_CUDA(cudaGetLastError());
+    ctx->launches += 4;
+    return HT_OK;
+}
+
+int ht_match_truth(ht_ctx *ctx, const ht_candidate *d_cand, uint32_t n_cand, const ht_truth *d_truth, uint32_t n_truth, double w_rho,
+                   double cos_w_phi, int32_t *d_cand_match, int32_t *d_truth_match, ht_match_summary *d_summary, void *cuda_stream)
+{
+    if (!ctx || !d_summary || !(w_rho >= 0.0) || !(cos_w_phi >= -1.0 && cos_w_phi <= 1.0)) return HT_ERR_INVALID_ARG;
+    if ((n_cand > 0 && (!d_cand || !d_cand_match)) || (n_truth > 0 && (!d_truth || !d_truth_match))) return HT_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    static_assert(sizeof(ht::TruthIn) == sizeof(ht_truth) && sizeof(ht::MatchSummary) == sizeof(ht_match_summary), "record layouts");
+    HT_CUDA(cudaMemsetAsync(d_summary, 0, sizeof(ht_match_summary), st));
+    const ht::CandOut *cd = reinterpret_cast<const ht::CandOut *>(d_cand);
+    const ht::TruthIn *tr = reinterpret_cast<const ht::TruthIn *>(d_truth);
+    ht::MatchSummary *sum = reinterpret_cast<ht::MatchSummary *>(d_summary);
+    const unsigned threads = 128;
+    if (n_cand > 0)
+        ht::match_candidates_kernel<<<(n_cand + threads - 1u) / threads, threads, 0, st>>>(cd, n_cand, tr, n_truth, ctx->geom, w_rho,
+                                                                                           cos_w_phi, d_cand_match);
+    if (n_truth > 0)
+        ht::match_truth_kernel<<<(n_truth + threads - 1u) / threads, threads, 0, st>>>(cd, n_cand, tr, n_truth, ctx->geom, w_rho,
+                                                                                       cos_w_phi, d_cand_match, d_truth_match, sum);
+    ht::match_summary_kernel<<<(std::max(n_cand, 1u) + threads - 1u) / threads, threads, 0, st>>>(d_cand_match, n_cand, n_truth, sum);
+    ht::match_finish_kernel<<<1, 1, 0, st>>>(sum);
+    HT_CUDA(cudaGetLastError());
+    ctx->launches += 4;
     return HT_OK;
 }
 

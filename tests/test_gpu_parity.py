@@ -591,6 +591,155 @@ def test_tracks_every_cell_of_a_small_odd_binning():
     assert tr["rho"][origin] == 0.0 and tr["phi"][origin] == 0.0
 
 
+# ------------------------------------------------------------------ f3: ridge merging and truth matching
+def _merge_gpu(g, pk, window, capacity=None):
+    dev = g.dev
+    n = len(pk)
+    rec = np.zeros((n, 3), np.uint32)
+    rec[:, 0], rec[:, 1], rec[:, 2] = pk["event"], pk["cell"], pk["count"]
+    d_pk = torch.from_numpy(rec.view(np.int32)).to(dev)
+    cap = n if capacity is None else capacity
+    d_out = torch.zeros(max(cap, 1) * 6, dtype=torch.int32, device=dev)
+    d_n = torch.full((1,), -5, dtype=torch.int32, device=dev)
+    nb = B.ht_merge_scratch_bytes(n)
+    d_scr = torch.empty(nb, dtype=torch.uint8, device=dev)
+    B.ht_merge_ridges(g.ctx, d_pk, n, window, d_out if cap else None, cap, d_n, d_scr, nb, None)
+    torch.cuda.synchronize()
+    found = int(d_n.cpu().numpy().view(np.uint32)[0])
+    k = min(found, cap)
+    out = d_out[:6 * k].cpu().numpy().view(np.uint8).view(B.CAND_DTYPE).copy()
+    return found, out[np.lexsort((out["cell"], out["event"]))], d_out
+
+
+def _check_merge(g, bn, pk, window):
+    from oracle import oracle_merge_ridges
+    want = oracle_merge_ridges(bn, pk, window)
+    found, got, _ = _merge_gpu(g, pk, window)
+    assert found == len(want)
+    for f in ("event", "cell", "count", "n_peaks"):
+        np.testing.assert_array_equal(got[f], want[f], err_msg=f)
+    np.testing.assert_allclose(got["rho"].astype(np.float64), want["rho"], rtol=2.4e-7, atol=0)
+    np.testing.assert_allclose(got["phi"].astype(np.float64), want["phi"], rtol=0, atol=6e-7)
+    return len(want)
+
+
+def test_ridge_merging_matches_the_oracle():
+    """Set-exact on (event, cell, count, members); rho, phi within the read-out's tolerance.  Peak lists of the tiny and of
+    the paper-shaped workload (in the fused kernel's own order), every window from 0 to 12, dense random lists with ties
+    and duplicate records, an empty list, and truncation of the candidate list."""
+    rng = np.random.default_rng(5)
+    for cfg_id, bn in ((1, WORKLOADS[1].binning), (2, Binning(4, 16, 256, 512))):
+        wl = WORKLOADS[cfg_id]
+        batch = generate_batch(wl, n_events=3)
+        with GpuHough(bn, 3, batch.n_hits) as g:
+            _, n, pk = g.fill_peaks(batch, wl.threshold, store=False)
+            assert n == len(pk) > 10
+            sizes = [_check_merge(g, bn, pk, w) for w in (0, 1, 2, 3, 5, 8, 12)]
+            assert sizes[0] == len(pk) and sizes == sorted(sizes, reverse=True) and sizes[-1] < sizes[0]
+            # truncation: the count is total, the written records are candidates of the full answer
+            found, part, _ = _merge_gpu(g, pk, 3, capacity=5)
+            from oracle import oracle_merge_ridges
+            full = oracle_merge_ridges(bn, pk, 3)
+            assert found == len(full) and len(part) == 5
+            keys = set(zip(full["event"].tolist(), full["cell"].tolist()))
+            assert all((int(e), int(c)) in keys for e, c in zip(part["event"], part["cell"]))
+            assert _merge_gpu(g, pk[:0], 3)[0] == 0
+    bn = Binning(2, 3, 40, 50)
+    with GpuHough(bn, 4, 1) as g:
+        for trial in range(6):
+            n = int(rng.integers(100, 1500))
+            keys = rng.choice(4 * bn.cells, size=n, replace=False)
+            pk = np.zeros(n, B.PEAK_DTYPE)
+            pk["event"], pk["cell"], pk["count"] = keys // bn.cells, keys % bn.cells, rng.integers(8, 11, n)
+            if trial % 2:
+                pk = np.concatenate([pk, pk[: n // 10]])            # duplicate records are linked at any window
+            for w in (0, 1, 4):
+                _check_merge(g, bn, pk, w)
+
+
+def test_truth_matching_matches_the_oracle():
+    """cand_match, truth_match and the integer part of the summary exactly (binary64 decisions by the same operations on both
+    sides), the residual sums within 1e-9 relative; on the paper-shaped event with the generator's truth and on random lists."""
+    from oracle import MERGED_DTYPE, TRUTH_DTYPE, oracle_match_truth, oracle_merge_ridges
+    from paper_1507_03074_b200.events import truth_table
+    import math
+
+    def run(g, bn, cand_gpu_tensor, n_cand, cand_oracle, tr, w_rho, w_phi):
+        dev = g.dev
+        d_tr = torch.from_numpy(tr.view(np.uint8).copy()).to(dev)
+        d_cm = torch.full((max(n_cand, 1),), -9, dtype=torch.int32, device=dev)
+        d_tm = torch.full((max(len(tr), 1),), -9, dtype=torch.int32, device=dev)
+        d_sum = torch.zeros(B.SUMMARY_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+        B.ht_match_truth(g.ctx, cand_gpu_tensor, n_cand, d_tr, len(tr), w_rho, math.cos(w_phi), d_cm, d_tm, d_sum, None)
+        torch.cuda.synchronize()
+        cm, tm = d_cm.cpu().numpy()[:n_cand], d_tm.cpu().numpy()[:len(tr)]
+        s = d_sum.cpu().numpy().view(B.SUMMARY_DTYPE)[0]
+        wcm, wtm, ws = oracle_match_truth(bn, cand_oracle, tr, w_rho, math.cos(w_phi))
+        np.testing.assert_array_equal(cm, wcm)
+        np.testing.assert_array_equal(tm, wtm)
+        for k in ("n_cand", "n_truth", "n_matched", "n_fake", "n_found", "n_duplicate"):
+            assert int(s[k]) == ws[k], k
+        for k in ("sum_drho", "sum_drho2", "sum_dphi", "sum_dphi2"):
+            assert abs(float(s[k]) - ws[k]) <= 1e-9 * max(1.0, abs(ws[k])) + 1e-12, k
+        return ws
+
+    wl = WORKLOADS[2]
+    bn = Binning(4, 16, 512, 512)
+    batch = generate_batch(wl, n_events=2)
+    tt = truth_table(batch)
+    tr = np.zeros(len(tt["event"]), TRUTH_DTYPE)
+    tr["event"], tr["a"], tr["b"] = tt["event"], tt["a"], tt["b"]
+    with GpuHough(bn, 2, batch.n_hits) as g:
+        _, n, pk = g.fill_peaks(batch, wl.threshold, store=False)
+        found, cands, d_cands = _merge_gpu(g, pk, 4)
+        # the device list in ITS order against the oracle on the same records in the same order
+        dev_order = d_cands[:6 * found].cpu().numpy().view(np.uint8).view(B.CAND_DTYPE)
+        co = np.zeros(found, MERGED_DTYPE)
+        for f in ("event", "cell", "count", "n_peaks"):
+            co[f] = dev_order[f]
+        for w_rho, w_phi in ((40.0, 0.02), (100.0, 0.05), (0.0, 0.0), (1e4, 3.0)):
+            ws = run(g, bn, d_cands, found, co, tr, w_rho, w_phi)
+        assert ws["n_found"] > 0
+        run(g, bn, d_cands, 0, co[:0], tr, 40.0, 0.02)
+        run(g, bn, d_cands, found, co, tr[:0], 40.0, 0.02)
+        # random candidates (cells anywhere) and random circles
+        rng = np.random.default_rng(11)
+        for trial in range(4):
+            nc, nt = int(rng.integers(50, 800)), int(rng.integers(10, 300))
+            rc = np.zeros(nc, B.CAND_DTYPE)
+            rc["event"], rc["cell"] = rng.integers(0, 2, nc), rng.integers(0, bn.cells, nc)
+            co = np.zeros(nc, MERGED_DTYPE)
+            co["event"], co["cell"] = rc["event"], rc["cell"]
+            rt = np.zeros(nt, TRUTH_DTYPE)
+            rt["event"] = rng.integers(0, 2, nt)
+            rt["a"], rt["b"] = rng.uniform(-4000, 4000, nt), rng.uniform(-4000, 4000, nt)
+            d_rc = torch.from_numpy(rc.view(np.uint8).copy()).to(g.dev)
+            run(g, bn, d_rc, nc, co, rt, 150.0, 0.08)
+
+
+def test_vote_loop_exactness_preconditions():
+    """The vote loop decides ONCE per hit whether the three-instruction quotients are exact; hits and
+    binnings that fail the test -- B_min = 0 or tiny, tiny and huge coordinates, 2y denormal -- take __fdiv_rn.  Both
+    branches must give the oracle's matrix bit for bit."""
+    rng = np.random.default_rng(77)
+    wl = WORKLOADS[1]
+    base = generate_batch(wl, n_events=1)
+    x, y, z = (v.copy() for v in base.event(0))
+    odd = np.array([[1e-19, 2e-19, 1.0], [3e-20, -1e-19, -1.0], [1e10, 2e10, 1e9], [-3e18, 1e18, 1.0], [40.0, 1e-40, 3.0],
+                    [1e-30, 50.0, 1.0], [60.0, -1e-25, 2.0], [0.0, 70.0, 5.0], [1e19, 1e-19, 1.0]], np.float32)
+    xyz = np.concatenate([np.stack([x, y, z], -1), odd]).astype(np.float32)
+    for bn in (Binning(4, 16, 64, 64, b_min=0.0, b_max=4000.0),                       # B_min = 0: the context fails the test
+               Binning(2, 4, 64, 96, b_min=-1e-12, b_max=3000.0),                     # tiny B_min
+               Binning(2, 4, 32, 64, a_min=-1e-15, a_max=1e-15, b_min=-1e-15, b_max=2e-15),   # everything tiny
+               Binning(1, 2, 48, 64, a_min=-1e19, a_max=1e19, b_min=-2e19, b_max=1e19),       # everything huge
+               Binning(4, 16, 128, 128)):
+        for scale in (1.0, 1e-17, 1e16):
+            ev = (xyz * np.float32(scale)).astype(np.float32) if scale != 1.0 else xyz
+            batch = batch_from_arrays([ev, ev[rng.permutation(len(ev))][: len(ev) // 2]])
+            _check_batch(bn, batch, 2)
+            _check_batch(bn, batch_from_arrays([ev]), 2)
+
+
 def test_seeded_random_shapes():
     """40 seeded random binnings / batch shapes (ragged tiles, rows shared by several warps, NB % 4 != 0, empty events,
     odd hit counts, partial angle ranges): matrix and peaks against the oracle, through all three call paths.
