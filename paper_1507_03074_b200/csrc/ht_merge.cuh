@@ -155,7 +155,7 @@ __global__ void merge_groups_kernel(const PeakOut *__restrict__ peaks, Geom g, c
 
 // ---- truth matching -----------------------------------------------------------------------------------------------------
 // Every decision is a binary64 comparison of values computed with the operations and in the order of SPEC.md section 6
-// (the library is built with --fmad=false: no contraction; sqrt is correctly rounded), so the matches equal the oracle's.
+// (the library is built with --fmad=false: no contraction; sqrt is correctly rounded), so the matches are reproducible bit for bit by any IEEE implementation of that text.
 
 struct Centre {
     double a, b, rho;
