@@ -101,8 +101,10 @@ typedef struct ht_tuning {
     int32_t fill_plain_stores;         /* 1: tiles leave with plain stores instead of bulk (TMA) stores */
     int32_t cooperative_launch;        /* 1: cudaLaunchCooperativeKernel (0: ordinary launch, programmatic dependent
                                           launch: the next call's prologue overlaps this call's tail) */
-    int32_t host_copy_input;           /* 1: ht_run_host / ht_submit_host copy the hits to the device (0: single events
-                                          are read by the kernel straight from the pinned block, zero-copy) */
+    int32_t host_zero_copy;            /* 1: the kernel of a single host event reads the hits straight from the pinned block
+                                          (zero-copy over PCIe; no copy call, lowest latency of ONE synchronous event);
+                                          0: one asynchronous copy per event on a second stream, which overlaps the previous
+                                          event's kernel (measured: 54 us per pipelined event against 71 us) */
     int32_t peaks_unroll;              /* 2, 4 or 8 independent 16-byte loads per thread of the peak scan (0: 2) */
     int32_t peaks_ctas_per_sm;         /* > 0: cap of the peak scan's resident CTAs per SM */
     int32_t fill_store_warps;          /* 1: one store warp queues every tile store; 2: one store warp per slab (0: chosen
@@ -244,8 +246,8 @@ HT_API int ht_match_truth(ht_ctx *ctx, const ht_candidate *d_cand, uint32_t n_ca
 /*
  * End-to-end call with HOST buffers (f4; needs cfg.host_slots >= 1; the transfer is "the dominant part" of
  * the paper's total time -- here only the hits (12 bytes each) and the compacted peak list cross PCIe).
- * Packs offsets and hits into one pinned block, which the kernel reads directly (one event: every hit is read exactly
- * once, zero-copy over PCIe) or which is copied to the device in one transfer (batches, ht_tuning.host_copy_input),
+ * Packs offsets and hits into one pinned block, which is copied to the device in one transfer (or, for one event with
+ * ht_tuning.host_zero_copy, read by the kernel directly: every hit is read exactly once),
  * runs ht_fill_peaks (or ht_fill + ht_peaks where that is unsupported) on the context's own matrices (events in groups
  * of host_slots) with the peak list and count written by the kernel straight into mapped pinned memory, and
  * synchronises.  h_out receives min(*h_n_found, capacity) records; capacity <= cfg.host_peak_capacity.
@@ -272,6 +274,20 @@ HT_API int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const fl
 HT_API int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y, const float *h_z, int32_t n_hits,
                           uint32_t threshold);
 HT_API int ht_wait_host(ht_ctx *ctx, int32_t slot, ht_peak *h_out, uint32_t capacity, uint32_t *h_n_found);
+
+/*
+ * A SEQUENCE of independent events from host memory, each through its own fused kernel (a0-a5), pipelined over the
+ * context's slots by the library itself (ht_submit_host / ht_wait_host in a loop: event k+1 is packed and launched and
+ * event k-1's peaks are copied out while event k's kernel runs):
+ *   h_x, h_y, h_z, h_event_offsets  as for ht_run_host (n_events + 1 offsets; each event at most cfg.max_hits hits)
+ *   h_out       n_events * capacity_per_event records: event e's list starts at h_out + e * capacity_per_event and holds
+ *               min(h_n_found[e], capacity_per_event, cfg.host_peak_capacity) records with `event` = e
+ *   h_n_found   n_events counts
+ * Synchronous: returns when every event has been collected.  No event may be in flight in a slot.
+ */
+HT_API int ht_run_host_events(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_z,
+                              const int32_t *h_event_offsets, int32_t n_events, uint32_t threshold, ht_peak *h_out,
+                              uint32_t capacity_per_event, uint32_t *h_n_found);
 
 /* Free everything the context owns (not a caller-owned workspace).  NULL is allowed.  (Defines no step of the method.) */
 HT_API void ht_destroy(ht_ctx *ctx);

@@ -30,7 +30,7 @@ SUMMARY_DTYPE = np.dtype([("n_cand", np.int64), ("n_truth", np.int64), ("n_match
 
 EXPORTS = ("ht_query_sizes", "ht_create", "ht_create_ex", "ht_fill", "ht_fill_peaks", "ht_fill_naive", "ht_peaks", "ht_tracks",
            "ht_merge_scratch_bytes", "ht_merge_ridges", "ht_match_truth",
-           "ht_run_host", "ht_submit_host", "ht_wait_host", "ht_destroy", "ht_strerror")                  # include/ht.h
+           "ht_run_host", "ht_run_host_events", "ht_submit_host", "ht_wait_host", "ht_destroy", "ht_strerror")                  # include/ht.h
 DIAG_EXPORTS = ("ht_tables_host", "ht_kernel_launches", "ht_launch_info", "ht_selftest_division", "ht_diag_memset",
                 "ht_diag_vote_rates")                                                                     # include/ht_diag.h
 DIAG_PATTERNS = ("red_random", "red_random_71", "red_no_conflict", "red_two_way", "red_same", "atom_random",
@@ -63,7 +63,7 @@ class ht_tuning(C.Structure):
     """How the work is organised on the device (include/ht.h); never changes a result.  All zero = defaults."""
     _fields_ = [("fill_batch_classification", C.c_int32), ("fill_slab_kb", C.c_int32),
                 ("fill_plain_stores", C.c_int32), ("cooperative_launch", C.c_int32),
-                ("host_copy_input", C.c_int32), ("peaks_unroll", C.c_int32), ("peaks_ctas_per_sm", C.c_int32),
+                ("host_zero_copy", C.c_int32), ("peaks_unroll", C.c_int32), ("peaks_ctas_per_sm", C.c_int32),
                 ("fill_store_warps", C.c_int32), ("reserved", C.c_int32 * 8)]
 
 
@@ -121,6 +121,8 @@ def load() -> C.CDLL:
     lib.ht_match_truth.argtypes = [vp, vp, u32, vp, u32, C.c_double, C.c_double, vp, vp, vp, vp]
     lib.ht_run_host.restype = C.c_int
     lib.ht_run_host.argtypes = [vp, vp, vp, vp, vp, i32, i32, u32, vp, u32, vp, vp]
+    lib.ht_run_host_events.restype = C.c_int
+    lib.ht_run_host_events.argtypes = [vp, vp, vp, vp, vp, i32, u32, vp, u32, vp]
     lib.ht_selftest_division.restype = C.c_int
     lib.ht_selftest_division.argtypes = [i32, C.c_uint64, C.c_uint64, C.POINTER(C.c_uint64)]
     lib.ht_kernel_launches.restype = C.c_int64
@@ -250,6 +252,14 @@ def ht_run_host(ctx, h_x, h_y, h_z, h_event_offsets, n_events: int, n_hits_total
     _check(load().ht_run_host(ctx, _ptr(h_x), _ptr(h_y), _ptr(h_z), _ptr(h_event_offsets), n_events, n_hits_total,
                               threshold, _ptr(h_out), capacity, C.addressof(n), _ptr(h_mh)), "ht_run_host")
     return n.value
+
+
+def ht_run_host_events(ctx, h_x, h_y, h_z, h_event_offsets, n_events: int, threshold: int, h_out, capacity_per_event: int,
+                       h_n_found) -> None:
+    """A sequence of events from HOST buffers, one fused kernel each, pipelined over the context's slots by the library.
+    ``h_out``: n_events * capacity_per_event peak records; ``h_n_found``: n_events uint32 counts."""
+    _check(load().ht_run_host_events(ctx, _ptr(h_x), _ptr(h_y), _ptr(h_z), _ptr(h_event_offsets), n_events, threshold,
+                                     _ptr(h_out), capacity_per_event, _ptr(h_n_found)), "ht_run_host_events")
 
 
 def ht_submit_host(ctx, slot: int, h_x, h_y, h_z, n_hits: int, threshold: int) -> None:

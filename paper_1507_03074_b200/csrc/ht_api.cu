@@ -738,7 +738,7 @@ int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y
     // One event whose hits the grid reads exactly once (mode 1): straight from the pinned block (zero-copy over PCIe);
     // otherwise one packed copy on the copy stream, which overlaps the kernel of the previous event.
     const FillPlan &pl = plan_fill(ctx, 1, n_hits, true);
-    const bool zero_copy = !ctx->tun.host_copy_input && pl.ok && pl.mode == 1;
+    const bool zero_copy = ctx->tun.host_zero_copy && pl.ok && pl.mode == 1;
     const unsigned char *in_base = sl.d_in_mapped;
     if (!zero_copy) {
         HT_CUDA(cudaMemcpyAsync(sl.d_in, sl.h_in, ib.bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
@@ -804,7 +804,7 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
     // input block [offsets | x | y | z], 16-byte aligned parts, packed in pinned memory: ONE host-to-device copy
     const InBlock ib = in_block(ctx, n_hits_total);
     const FillPlan &pl1 = plan_fill(ctx, 1, n_hits_total, true);
-    const bool zero_copy = n_events == 1 && !ctx->tun.host_copy_input && pl1.ok && pl1.mode == 1;
+    const bool zero_copy = n_events == 1 && ctx->tun.host_zero_copy && pl1.ok && pl1.mode == 1;
     const unsigned char *in_base = zero_copy ? sl.d_in_mapped : sl.d_in;
     if (n_hits_total > 0) {
         const size_t nb = sizeof(float) * (size_t)n_hits_total;
@@ -846,6 +846,49 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
     }
     *h_n_found = found_total;
     return HT_OK;
+}
+
+int ht_run_host_events(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_z, const int32_t *h_event_offsets,
+                       int32_t n_events, uint32_t threshold, ht_peak *h_out, uint32_t capacity_per_event, uint32_t *h_n_found)
+{
+    if (!ctx || !h_n_found || n_events < 0) return HT_ERR_INVALID_ARG;
+    if (ctx->cfg.host_slots < 1) return HT_ERR_UNSUPPORTED;
+    if (n_events == 0) return HT_OK;
+    if (!h_event_offsets || threshold < 1u || (capacity_per_event > 0 && !h_out)) return HT_ERR_INVALID_ARG;
+    if (h_event_offsets[0] != 0) return HT_ERR_INVALID_ARG;
+    for (int e = 0; e < n_events; ++e) {
+        const int64_t n = (int64_t)h_event_offsets[e + 1] - h_event_offsets[e];
+        if (n < 0 || n > ctx->cfg.max_hits) return HT_ERR_INVALID_ARG;
+    }
+    if (h_event_offsets[n_events] > 0 && (!h_x || !h_y || !h_z)) return HT_ERR_INVALID_ARG;
+    for (const HostSlot &s : ctx->slots)
+        if (s.busy) return HT_ERR_INVALID_ARG;                    // submitted events must be waited for first
+    const int slots = ctx->cfg.host_slots;
+    auto collect = [&](int e) -> int {                            // event e sits in slot e % slots
+        ht_peak *dst = h_out ? h_out + (size_t)e * capacity_per_event : nullptr;
+        const int rc = ht_wait_host(ctx, e % slots, dst, capacity_per_event, &h_n_found[e]);
+        if (rc != HT_OK) return rc;
+        const uint32_t got = h_n_found[e] < capacity_per_event ? h_n_found[e] : capacity_per_event;
+        const uint32_t kept = got < ctx->cfg.host_peak_capacity ? got : ctx->cfg.host_peak_capacity;
+        for (uint32_t k = 0; k < kept; ++k) dst[k].event = (uint32_t)e;
+        return HT_OK;
+    };
+    int rc = HT_OK, collected = 0;
+    for (int e = 0; e < n_events && rc == HT_OK; ++e) {
+        if (e - collected == slots) rc = collect(collected++);    // the slot's previous event (submitted `slots` events ago)
+        if (rc != HT_OK) break;
+        const int32_t lo = h_event_offsets[e], n = h_event_offsets[e + 1] - lo;
+        rc = ht_submit_host(ctx, e % slots, h_x ? h_x + lo : nullptr, h_y ? h_y + lo : nullptr, h_z ? h_z + lo : nullptr, n, threshold);
+        if (rc != HT_OK) {                                        // leave no event in flight
+            for (; collected < e; ++collected) collect(collected);
+            return rc;
+        }
+    }
+    for (; collected < n_events; ++collected) {
+        const int r2 = collect(collected);
+        if (rc == HT_OK) rc = r2;
+    }
+    return rc;
 }
 
 int ht_tracks(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, ht_track *d_out, void *cuda_stream)

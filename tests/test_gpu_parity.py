@@ -399,7 +399,7 @@ def test_submit_wait_host_pipeline():
     bn = Binning(4, 16, 256, 256)
     events = [generate_batch(wl, n_events=1, first_event=e) for e in range(7)]
     wants = [oracle_peaks(bn, oracle_fill(bn, *b.event(0))[0], wl.threshold) for b in events]
-    for tuning in (None, {"host_copy_input": 1}):
+    for tuning in (None, {"host_zero_copy": 1}):
         with GpuHough(bn, 1, 6000, host_slots=3, host_peak_capacity=4096, tuning=tuning) as g:
             out = np.zeros(4096, B.PEAK_DTYPE)
             in_flight = {}
@@ -526,7 +526,7 @@ def test_run_host_single_event_zero_copy_and_copy(copy_input):
     copied to the device first; same matrix, same peaks, several calls in a row on one context."""
     wl = WORKLOADS[2]
     bn = Binning(4, 16, 256, 256)
-    with GpuHough(bn, 1, 6000, host_slots=1, host_peak_capacity=8192, tuning={"host_copy_input": copy_input}) as g:
+    with GpuHough(bn, 1, 6000, host_slots=1, host_peak_capacity=8192, tuning={"host_zero_copy": copy_input}) as g:
         for ev in range(3):
             batch = generate_batch(wl, n_events=1, first_event=ev)
             want_m = _oracle_batch(bn, batch)
@@ -538,6 +538,45 @@ def test_run_host_single_event_zero_copy_and_copy(copy_input):
             assert n == len(want) and n > 0
             np.testing.assert_array_equal(sort_peaks(out[:n], bn.cells), want)
             np.testing.assert_array_equal(h_mh.reshape(want_m[0].shape), want_m[0])
+
+
+def test_run_host_events_pipelines_a_sequence():
+    """ht_run_host_events: a sequence of ragged events (an empty one among them) from host memory, one fused kernel each,
+    pipelined over 1, 2 and 3 slots, with and without zero-copy input: every event's peak list equals the oracle's; lists
+    longer than capacity_per_event are truncated, their counts are not."""
+    wl = WORKLOADS[2]
+    bn = Binning(4, 16, 256, 256)
+    evs = []
+    for e in range(7):
+        b = generate_batch(WORKLOADS[3], n_events=1, first_event=e)
+        evs.append(np.stack(b.event(0), -1)[: 1200 + 300 * e])
+    evs.insert(3, np.zeros((0, 3), np.float32))
+    batch = batch_from_arrays(evs)
+    wants = [oracle_peaks(bn, oracle_fill(bn, *batch.event(e))[0], wl.threshold) for e in range(batch.n_events)]
+    assert max(len(w) for w in wants) > 20 and len(wants[3]) == 0
+    for slots, tuning in ((1, None), (2, {"host_zero_copy": 1}), (3, None)):
+        with GpuHough(bn, 1, 4000, host_slots=slots, host_peak_capacity=4096, tuning=tuning) as g:
+            for cap_ev in (4096, 16):
+                out = np.zeros(batch.n_events * cap_ev, B.PEAK_DTYPE)
+                nf = np.zeros(batch.n_events, np.uint32)
+                B.ht_run_host_events(g.ctx, batch.x, batch.y, batch.z, batch.event_offsets, batch.n_events, wl.threshold,
+                                     out, cap_ev, nf)
+                for e, want in enumerate(wants):
+                    assert nf[e] == len(want), (slots, e)
+                    got = out[e * cap_ev: e * cap_ev + min(len(want), cap_ev)]
+                    assert np.all(got["event"] == e)
+                    if len(want) <= cap_ev:
+                        got = got[np.argsort(got["cell"])]
+                        np.testing.assert_array_equal(got["cell"], want["cell"])
+                        np.testing.assert_array_equal(got["count"], want["count"])
+                    else:
+                        keys = dict(zip(want["cell"].tolist(), want["count"].tolist()))
+                        assert len(set(got["cell"].tolist())) == cap_ev
+                        assert all(keys.get(int(c)) == int(n) for c, n in zip(got["cell"], got["count"]))
+            # an event beyond the context's capacity is refused before anything is launched
+            with pytest.raises(B.HtError):
+                big = batch_from_arrays([np.ones((4001, 3), np.float32)])
+                B.ht_run_host_events(g.ctx, big.x, big.y, big.z, big.event_offsets, 1, wl.threshold, out, 16, nf)
 
 
 # ------------------------------------------------------------------ f3: track read-out of the peaks
