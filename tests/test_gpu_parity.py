@@ -322,7 +322,7 @@ def test_fused_kernel_list_truncation():
             assert n2 == len(want) and len(got2) == len(want) - 1 and got2 <= full
 
 
-@pytest.mark.parametrize("tuning", [None, {"fill_batch_classification": 1}, {"cooperative_launch": 1}])
+@pytest.mark.parametrize("tuning", [None, {"fill_batch_classification": 1}, {"cooperative_launch": 1}, {"fill_store_warps": 2}])
 def test_repeated_launches_give_the_same_bits(tuning):
     """No timing-dependent result: 3000 back-to-back fused launches per variant (hand-rolled grid barrier, named-barrier
     pipeline, TMA proxy fence, dependent launches overlapping their predecessor's tail), matrix and peak set compared on
