@@ -101,10 +101,10 @@ typedef struct ht_tuning {
     int32_t fill_plain_stores;         /* 1: tiles leave with plain stores instead of bulk (TMA) stores */
     int32_t cooperative_launch;        /* 1: cudaLaunchCooperativeKernel (0: ordinary launch, programmatic dependent
                                           launch: the next call's prologue overlaps this call's tail) */
-    int32_t host_zero_copy;            /* 1: the kernel of a single host event reads the hits straight from the pinned block
-                                          (zero-copy over PCIe; no copy call, lowest latency of ONE synchronous event);
-                                          0: one asynchronous copy per event on a second stream, which overlaps the previous
-                                          event's kernel (measured: 54 us per pipelined event against 71 us) */
+    int32_t host_copy_input;           /* 0: the kernel of a single host event reads the hits straight from the pinned block
+                                          (zero-copy over PCIe, coalesced; no copy call and no event between two kernels of
+                                          the stream, so consecutive events keep their dependent launch: 52 us per pipelined
+                                          event); 1: one asynchronous copy per event on a second stream (56 us) */
     int32_t peaks_unroll;              /* 2, 4 or 8 independent 16-byte loads per thread of the peak scan (0: 2) */
     int32_t peaks_ctas_per_sm;         /* > 0: cap of the peak scan's resident CTAs per SM */
     int32_t fill_store_warps;          /* 1: one store warp queues every tile store; 2: one store warp per slab (0: chosen
@@ -246,8 +246,8 @@ HT_API int ht_match_truth(ht_ctx *ctx, const ht_candidate *d_cand, uint32_t n_ca
 /*
  * End-to-end call with HOST buffers (f4; needs cfg.host_slots >= 1; the transfer is "the dominant part" of
  * the paper's total time -- here only the hits (12 bytes each) and the compacted peak list cross PCIe).
- * Packs offsets and hits into one pinned block, which is copied to the device in one transfer (or, for one event with
- * ht_tuning.host_zero_copy, read by the kernel directly: every hit is read exactly once),
+ * Packs offsets and hits into one pinned block, which the kernel reads directly (one event: every hit is read exactly
+ * once, zero-copy over PCIe) or which is copied to the device in one transfer (batches, ht_tuning.host_copy_input),
  * runs ht_fill_peaks (or ht_fill + ht_peaks where that is unsupported) on the context's own matrices (events in groups
  * of host_slots) with the peak list and count written by the kernel straight into mapped pinned memory, and
  * synchronises.  h_out receives min(*h_n_found, capacity) records; capacity <= cfg.host_peak_capacity.

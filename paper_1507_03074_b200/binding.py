@@ -63,7 +63,7 @@ class ht_tuning(C.Structure):
     """How the work is organised on the device (include/ht.h); never changes a result.  All zero = defaults."""
     _fields_ = [("fill_batch_classification", C.c_int32), ("fill_slab_kb", C.c_int32),
                 ("fill_plain_stores", C.c_int32), ("cooperative_launch", C.c_int32),
-                ("host_zero_copy", C.c_int32), ("peaks_unroll", C.c_int32), ("peaks_ctas_per_sm", C.c_int32),
+                ("host_copy_input", C.c_int32), ("peaks_unroll", C.c_int32), ("peaks_ctas_per_sm", C.c_int32),
                 ("fill_store_warps", C.c_int32), ("reserved", C.c_int32 * 8)]
 
 

@@ -8,6 +8,7 @@
 #include "ht_merge.cuh"
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -173,6 +174,8 @@ struct HostSlot {
     unsigned char *h_res = nullptr, *d_res = nullptr;                          // mapped pinned result block and its device alias
     cudaEvent_t copied = nullptr, done = nullptr;
     bool busy = false;
+    uint32_t seq = 0;                  // number of the slot's last submission (the kernel writes it into the result header)
+    bool flagged = false;              // completion is signalled by the kernel through the header, not by `done`
 };
 
 }  // namespace
@@ -367,6 +370,7 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
             return fail(cuda_fail(e, "cudaHostAlloc(input)"));
         if ((e = cudaHostAlloc((void **)&ctx->h_res_all, lay.res_block * ns, cudaHostAllocMapped)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaHostAlloc(result)"));
+        std::memset(ctx->h_res_all, 0, lay.res_block * ns);          // (the completion word of a slot starts at 0, its first submission is number 1)
         unsigned char *in_map = nullptr, *res_map = nullptr;
         if ((e = cudaHostGetDevicePointer((void **)&in_map, ctx->h_in_all, 0)) != cudaSuccess ||
             (e = cudaHostGetDevicePointer((void **)&res_map, ctx->h_res_all, 0)) != cudaSuccess)
@@ -496,7 +500,7 @@ const FillPlan &plan_fill(ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool pe
 // pinned staging blocks), so the kernel may read them before the previous kernel of the stream has completed.
 int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off, int32_t n_events,
                 int32_t n_hits_total, uint32_t *d_mh, bool peaks, uint32_t threshold, ht_peak *d_out, uint32_t capacity,
-                uint32_t *d_n_found, cudaStream_t st, bool early_inputs)
+                uint32_t *d_n_found, cudaStream_t st, bool early_inputs, uint32_t *d_done_flag = nullptr, uint32_t done_value = 0u)
 {
     const ht::Geom &g = ctx->geom;
     const FillPlan &pl = plan_fill(ctx, n_events, n_hits_total, peaks);
@@ -535,6 +539,8 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.mh = d_mh;
     a.bulk_ok = (g.n_b % 4 == 0) && ((reinterpret_cast<uintptr_t>(d_mh) & 15u) == 0) && !ctx->tun.fill_plain_stores;
     a.early_inputs = early_inputs ? 1 : 0;
+    a.done_flag = d_done_flag;
+    a.done_value = done_value;
     a.threshold = threshold;
     static_assert(sizeof(ht::PeakOut) == sizeof(ht_peak), "peak record layout");
     a.out = reinterpret_cast<ht::PeakOut *>(d_out);
@@ -692,7 +698,7 @@ InBlock in_block(const ht_ctx *ctx, int32_t n_hits)
 // One group of events (at most host_slots, all in the input block of slot `s`, matrices from `mh_slot` on) through the
 // fused kernel (or the two-call path for shapes it refuses), peak list and count into slot s's mapped result block.
 int enqueue_group(ht_ctx *ctx, HostSlot &sl, const unsigned char *in_base, const InBlock &ib, int32_t hit_base, int32_t ne,
-                  int32_t nh, uint32_t *d_mh, uint32_t threshold, uint32_t room, bool early_inputs)
+                  int32_t nh, uint32_t *d_mh, uint32_t threshold, uint32_t room, bool early_inputs, bool flag = false)
 {
     cudaStream_t st = ctx->host_stream;
     const float *d_x = reinterpret_cast<const float *>(in_base + ib.o_x) + hit_base;
@@ -701,8 +707,12 @@ int enqueue_group(ht_ctx *ctx, HostSlot &sl, const unsigned char *in_base, const
     const int32_t *d_off = reinterpret_cast<const int32_t *>(in_base);
     uint32_t *d_count = reinterpret_cast<uint32_t *>(sl.d_res);
     ht_peak *d_list = reinterpret_cast<ht_peak *>(sl.d_res + kResHeader);
-    int rc = launch_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, true, threshold, d_list, room, d_count, st, early_inputs);
+    // the kernel itself tells the host when the results are in the mapped block (second word of the header)
+    sl.flagged = flag;
+    int rc = launch_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, true, threshold, d_list, room, d_count, st, early_inputs,
+                         flag ? d_count + 1 : nullptr, sl.seq);
     if (rc == HT_ERR_UNSUPPORTED) {
+        sl.flagged = false;
         rc = ht_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, st);
         if (rc == HT_ERR_UNSUPPORTED) rc = ht_fill_naive(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, st);
         if (rc != HT_OK) return rc;
@@ -738,7 +748,7 @@ int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y
     // One event whose hits the grid reads exactly once (mode 1): straight from the pinned block (zero-copy over PCIe);
     // otherwise one packed copy on the copy stream, which overlaps the kernel of the previous event.
     const FillPlan &pl = plan_fill(ctx, 1, n_hits, true);
-    const bool zero_copy = ctx->tun.host_zero_copy && pl.ok && pl.mode == 1;
+    const bool zero_copy = !ctx->tun.host_copy_input && pl.ok && pl.mode == 1;
     const unsigned char *in_base = sl.d_in_mapped;
     if (!zero_copy) {
         HT_CUDA(cudaMemcpyAsync(sl.d_in, sl.h_in, ib.bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
@@ -747,9 +757,12 @@ int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y
         in_base = sl.d_in;
     }
     uint32_t *d_mh = ctx->d_hmh + (size_t)slot * (size_t)ctx->geom.cells;
-    const int rc = enqueue_group(ctx, sl, in_base, ib, 0, 1, n_hits, d_mh, threshold, ctx->cfg.host_peak_capacity, true);
+    ++sl.seq;
+    const int rc = enqueue_group(ctx, sl, in_base, ib, 0, 1, n_hits, d_mh, threshold, ctx->cfg.host_peak_capacity, true, true);
     if (rc != HT_OK) return rc;
-    HT_CUDA(cudaEventRecord(sl.done, ctx->host_stream));
+    // (no event between two kernels of the stream when the kernel signals its own completion: an event record there
+    // would undo the dependent launch of the next one)
+    if (!sl.flagged) HT_CUDA(cudaEventRecord(sl.done, ctx->host_stream));
     sl.busy = true;
     return HT_OK;
 }
@@ -762,7 +775,19 @@ int ht_wait_host(ht_ctx *ctx, int32_t slot, ht_peak *h_out, uint32_t capacity, u
     HostSlot &sl = ctx->slots[(size_t)slot];
     if (!sl.busy) return HT_ERR_INVALID_ARG;
     DeviceGuard guard(ctx->cfg.device);
-    HT_CUDA(cudaEventSynchronize(sl.done));
+    if (sl.flagged) {
+        const volatile uint32_t *flag = reinterpret_cast<const volatile uint32_t *>(sl.h_res) + 1;
+        for (uint32_t spins = 0; *flag != sl.seq; ++spins) {
+            if ((spins & 0xFFFu) == 0xFFFu) {                     // a failed kernel never writes the flag
+                const cudaError_t q = cudaStreamQuery(ctx->host_stream);
+                if (q != cudaSuccess && q != cudaErrorNotReady) return cuda_fail(q, "ht_wait_host");
+                if (q == cudaSuccess && *flag != sl.seq) return cuda_fail(cudaErrorUnknown, "ht_wait_host: stream idle, no result");
+            }
+        }
+        std::atomic_thread_fence(std::memory_order_acquire);
+    } else {
+        HT_CUDA(cudaEventSynchronize(sl.done));
+    }
     sl.busy = false;
     const uint32_t found = *reinterpret_cast<const volatile uint32_t *>(sl.h_res);
     uint32_t got = found < ctx->cfg.host_peak_capacity ? found : ctx->cfg.host_peak_capacity;
@@ -804,7 +829,7 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
     // input block [offsets | x | y | z], 16-byte aligned parts, packed in pinned memory: ONE host-to-device copy
     const InBlock ib = in_block(ctx, n_hits_total);
     const FillPlan &pl1 = plan_fill(ctx, 1, n_hits_total, true);
-    const bool zero_copy = n_events == 1 && ctx->tun.host_zero_copy && pl1.ok && pl1.mode == 1;
+    const bool zero_copy = n_events == 1 && !ctx->tun.host_copy_input && pl1.ok && pl1.mode == 1;
     const unsigned char *in_base = zero_copy ? sl.d_in_mapped : sl.d_in;
     if (n_hits_total > 0) {
         const size_t nb = sizeof(float) * (size_t)n_hits_total;

@@ -399,7 +399,7 @@ def test_submit_wait_host_pipeline():
     bn = Binning(4, 16, 256, 256)
     events = [generate_batch(wl, n_events=1, first_event=e) for e in range(7)]
     wants = [oracle_peaks(bn, oracle_fill(bn, *b.event(0))[0], wl.threshold) for b in events]
-    for tuning in (None, {"host_zero_copy": 1}):
+    for tuning in (None, {"host_copy_input": 1}):
         with GpuHough(bn, 1, 6000, host_slots=3, host_peak_capacity=4096, tuning=tuning) as g:
             out = np.zeros(4096, B.PEAK_DTYPE)
             in_flight = {}
@@ -526,7 +526,7 @@ def test_run_host_single_event_zero_copy_and_copy(copy_input):
     copied to the device first; same matrix, same peaks, several calls in a row on one context."""
     wl = WORKLOADS[2]
     bn = Binning(4, 16, 256, 256)
-    with GpuHough(bn, 1, 6000, host_slots=1, host_peak_capacity=8192, tuning={"host_zero_copy": copy_input}) as g:
+    with GpuHough(bn, 1, 6000, host_slots=1, host_peak_capacity=8192, tuning={"host_copy_input": copy_input}) as g:
         for ev in range(3):
             batch = generate_batch(wl, n_events=1, first_event=ev)
             want_m = _oracle_batch(bn, batch)
@@ -554,7 +554,7 @@ def test_run_host_events_pipelines_a_sequence():
     batch = batch_from_arrays(evs)
     wants = [oracle_peaks(bn, oracle_fill(bn, *batch.event(e))[0], wl.threshold) for e in range(batch.n_events)]
     assert max(len(w) for w in wants) > 20 and len(wants[3]) == 0
-    for slots, tuning in ((1, None), (2, {"host_zero_copy": 1}), (3, None)):
+    for slots, tuning in ((1, None), (2, {"host_copy_input": 1}), (3, None)):
         with GpuHough(bn, 1, 4000, host_slots=slots, host_peak_capacity=4096, tuning=tuning) as g:
             for cap_ev in (4096, 16):
                 out = np.zeros(batch.n_events * cap_ev, B.PEAK_DTYPE)
