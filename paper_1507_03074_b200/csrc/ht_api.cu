@@ -225,7 +225,7 @@ namespace {
 size_t fill_smem_bytes(const ht_config &c, long long rows, int mode, long long n_hits)
 {
     const size_t slab = align_up((size_t)rows * (size_t)c.n_b * 4u, 16);
-    size_t b = 2u * slab + 8u * 4u * (size_t)(rows + 4);     // two slabs, two_a[8 ring entries][rows + 4]
+    size_t b = 2u * slab + 8u * 4u * (size_t)((rows + 7) & ~3ll);     // two slabs, two_a[8 ring entries][rows + 4, rounded up to 4]
     if (mode == 1) b += 4u * (size_t)c.n_theta * (size_t)c.n_phi;            // hits per plane
     (void)n_hits;
     return align_up(b, 16);
