@@ -948,7 +948,7 @@ int ht_merge_ridges(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, uint3
     if (ro != HT_OK) return ro;
     const int planes_all = ctx->cfg.n_theta * ctx->cfg.n_phi;
     const unsigned long long groups = (unsigned long long)ctx->cfg.max_events * (unsigned long long)planes_all;
-    if (groups >= (1ull << 31)) return HT_ERR_UNSUPPORTED;
+    if (groups >= (1ull << 31) || ctx->cfg.n_a > 65535 || ctx->cfg.n_b > 65535) return HT_ERR_UNSUPPORTED;   // (a, b) packed in 32 bits
     uint32_t *slot = static_cast<uint32_t *>(d_scratch), *order = slot + n_peaks, *label = order + n_peaks;
     const ht::PeakOut *pk = reinterpret_cast<const ht::PeakOut *>(d_peaks);
     const unsigned threads = 256, blocks = (n_peaks + threads - 1u) / threads;
@@ -956,7 +956,7 @@ int ht_merge_ridges(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, uint3
                                                        ctx->d_counts, slot);
     ht::merge_scan_kernel<<<1, 1024, 0, st>>>(ctx->d_counts, ctx->d_bucket_start, (uint32_t)groups);
     ht::merge_scatter_kernel<<<blocks, threads, 0, st>>>(pk, n_peaks, ctx->geom, planes_all, ctx->d_bucket_start, slot, order);
-    ht::merge_groups_kernel<<<(unsigned)groups, 128, 0, st>>>(pk, ctx->geom, ctx->d_bucket_start, order, label, window,
+    ht::merge_groups_kernel<<<(unsigned)groups, ht::kMergeThreads, 0, st>>>(pk, ctx->geom, ctx->d_bucket_start, order, label, window,
                                                               reinterpret_cast<ht::CandOut *>(d_out), capacity, d_n_out);
     HT_CUDA(cudaGetLastError());
     ctx->launches += 4;

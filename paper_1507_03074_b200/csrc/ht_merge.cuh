@@ -97,33 +97,56 @@ __global__ void merge_scatter_kernel(const PeakOut *__restrict__ peaks, uint32_t
     order[(uint32_t)start[group_of_peak(peaks[i], g, planes_all)] + slot[i]] = i;
 }
 
-// one CTA per (event, plane) group; order[] holds the peaks of group k at [start[k], start[k+1]); label[] is scratch
-__global__ void merge_groups_kernel(const PeakOut *__restrict__ peaks, Geom g, const int32_t *__restrict__ start,
-                                    const uint32_t *__restrict__ order, uint32_t *label, uint32_t window,
-                                    CandOut *__restrict__ out, uint32_t capacity, uint32_t *n_out)
+// one CTA per (event, plane) group; order[] holds the peaks of group k at [start[k], start[k+1]); label[] is scratch.
+// Groups of up to kMergeSmem peaks keep their (a, b) cells and labels in shared memory (the pair loop reads them m times
+// per sweep); larger groups work on global memory.
+constexpr int kMergeThreads = 256;
+constexpr int kMergeSmem = 2048;
+
+__global__ void __launch_bounds__(kMergeThreads)
+merge_groups_kernel(const PeakOut *__restrict__ peaks, Geom g, const int32_t *__restrict__ start,
+                    const uint32_t *__restrict__ order, uint32_t *label_global, uint32_t window,
+                    CandOut *__restrict__ out, uint32_t capacity, uint32_t *n_out)
 {
+    __shared__ uint32_t s_ab[kMergeSmem];                               // a << 16 | b  (both < 65536: checked by the host)
+    __shared__ uint32_t s_label[kMergeSmem];
     const int lo = start[blockIdx.x], hi = start[blockIdx.x + 1];
     const int m = hi - lo;
     if (m <= 0) return;
     const uint32_t NB = (uint32_t)g.n_b, NA = (uint32_t)g.n_a;
-    auto a_of = [&](uint32_t cell) { return (int)((cell / NB) % NA); };
-    auto b_of = [&](uint32_t cell) { return (int)(cell % NB); };
-    for (int i = threadIdx.x; i < m; i += blockDim.x) label[lo + i] = (uint32_t)i;
+    const bool in_smem = m <= kMergeSmem;
+    uint32_t *label = in_smem ? s_label : label_global + lo;
+    auto ab_of = [&](int i) -> uint32_t {
+        if (in_smem) return s_ab[i];
+        const uint32_t cell = peaks[order[lo + i]].cell;
+        return (((cell / NB) % NA) << 16) | (cell % NB);
+    };
+    for (int i = threadIdx.x; i < m; i += blockDim.x) {
+        label[i] = (uint32_t)i;
+        if (in_smem) {
+            const uint32_t cell = peaks[order[lo + i]].cell;
+            s_ab[i] = (((cell / NB) % NA) << 16) | (cell % NB);
+        }
+    }
     __syncthreads();
     for (;;) {
         int changed = 0;
         for (int i = threadIdx.x; i < m; i += blockDim.x) {
-            const uint32_t ci = peaks[order[lo + i]].cell;
-            const int ai = a_of(ci), bi = b_of(ci);
-            uint32_t l = *reinterpret_cast<volatile uint32_t *>(&label[lo + i]);
+            const uint32_t abi = ab_of(i);
+            const int ai = (int)(abi >> 16), bi = (int)(abi & 0xFFFFu);
+            uint32_t l = *reinterpret_cast<volatile uint32_t *>(&label[i]);
             const uint32_t l0 = l;
             for (int j = 0; j < m; ++j) {
-                const uint32_t cj = peaks[order[lo + j]].cell;
-                const int da = abs(ai - a_of(cj)), db = abs(bi - b_of(cj));
-                if ((uint32_t)max(da, db) <= window) l = min(l, *reinterpret_cast<volatile uint32_t *>(&label[lo + j]));
+                const uint32_t abj = ab_of(j);
+                const int da = abs(ai - (int)(abj >> 16)), db = abs(bi - (int)(abj & 0xFFFFu));
+                if ((uint32_t)max(da, db) <= window) l = min(l, *reinterpret_cast<volatile uint32_t *>(&label[j]));
             }
+            // follow the labels down to their current root (a label is a position of the same component, never larger
+            // than the position that holds it): long ridges converge in a few sweeps instead of one per link
+            for (uint32_t up = *reinterpret_cast<volatile uint32_t *>(&label[l]); up < l;
+                 up = *reinterpret_cast<volatile uint32_t *>(&label[l])) l = up;
             if (l < l0) {
-                atomicMin(&label[lo + i], l);
+                atomicMin(&label[i], l);
                 changed = 1;
             }
         }
@@ -131,19 +154,20 @@ __global__ void merge_groups_kernel(const PeakOut *__restrict__ peaks, Geom g, c
     }
     // roots (label == own position) emit their component
     for (int i = threadIdx.x; i < m; i += blockDim.x) {
-        if (label[lo + i] != (uint32_t)i) continue;
+        if (label[i] != (uint32_t)i) continue;
         uint32_t members = 0u;
         PeakOut best = peaks[order[lo + i]];
         for (int j = 0; j < m; ++j) {
-            if (label[lo + j] != (uint32_t)i) continue;
+            if (label[j] != (uint32_t)i) continue;
             ++members;
             const PeakOut p = peaks[order[lo + j]];
             if (p.count > best.count || (p.count == best.count && p.cell < best.cell)) best = p;
         }
         const uint32_t at = atomicAdd(n_out, 1u);
         if (at < capacity) {
-            const float A = __fadd_rn(g.a_min, __fmul_rn(__fadd_rn((float)a_of(best.cell), 0.5f), g.dA));   // bin centres (R5, R18)
-            const float B = __fadd_rn(g.b_min, __fmul_rn(__fadd_rn((float)b_of(best.cell), 0.5f), g.dB));
+            const uint32_t ia = (best.cell / NB) % NA, ib = best.cell % NB;
+            const float A = __fadd_rn(g.a_min, __fmul_rn(__fadd_rn((float)ia, 0.5f), g.dA));   // bin centres (R5, R18)
+            const float B = __fadd_rn(g.b_min, __fmul_rn(__fadd_rn((float)ib, 0.5f), g.dB));
             CandOut c;
             c.event = best.event; c.cell = best.cell; c.count = best.count; c.n_peaks = members;
             c.rho = __fsqrt_rn(__fadd_rn(__fmul_rn(A, A), __fmul_rn(B, B)));
