@@ -55,11 +55,16 @@ def measured_hbm_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def workload_config(wl, n_hits, n_ev):
-    """The `config` block both arms print (same keys, same values for the same workload)."""
+def workload_config(wl, n_hits, n_ev, steps, reps):
+    """The `config` block: BOTH arms print exactly this dict (same keys, same values) for the same workload and flags."""
     bn = wl.binning
+    m_bytes = 4 * bn.cells * n_ev
     return {"workload": f"config{wl.config}:{wl.name}", "bins": [bn.n_theta, bn.n_phi, bn.n_a, bn.n_b],
-            "hits_per_step": int(n_hits), "events_per_step": int(n_ev), "threshold": int(wl.threshold)}
+            "hits_per_step": int(n_hits), "events_per_step": int(n_ev), "threshold": int(wl.threshold),
+            "l2": f"M_H per step ({m_bytes / 1e6:.0f} MB) is larger than the 126 MB L2, and the CUDA arm rotates its output "
+                  "matrices, so no step inherits another step's lines",
+            "launch_mode": f"CUDA arm: plain stream launches (fixed rule), median of {reps} brackets of exactly {steps} calls each; "
+                           "reference arm: the CPU oracle as it stands, one thread, the steps timed in one bracket"}
 
 
 class ClockSampler(threading.Thread):
@@ -170,7 +175,7 @@ def bench_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": DTYPE, "data": "synthetic",
-        "config": workload_config(wl, batch.n_hits, n_ev),
+        "config": workload_config(wl, batch.n_hits, n_ev, args.steps, args.reps),
         "votes_per_s": votes * args.steps / total,
         "cpu_baseline": {"value": value, "unit": "events/s", "cores": 1, "kind": "oracle",
                          "sample": f"{args.steps} steps of {n_ev} full event(s) of this workload, single thread"},
@@ -560,22 +565,20 @@ def bench_ours(args):
         vote_roof["frac_of_slowest_bound"] = vote_roof["bound_us"] / (ms_per_step * 1e3)
 
         info = B.ht_launch_info(ctx)
-        config = workload_config(wl, n_hits, n_ev)
-        config.update({
+        config = workload_config(wl, n_hits, n_ev, K, R)
+        detail = {
             "path": ("ht_fill_peaks: one kernel does a0-a5 and stores every M_H cell once" if headline == "fused"
                      else "ht_fill + ht_peaks (two kernels)"),
-            "l2": f"M_H per step ({m_bytes / 1e6:.0f} MB) is larger than the 126 MB L2; {n_rot} output matrices "
-                  "rotated so no step inherits another step's lines",
+            "rotated_output_matrices": n_rot,
             "launch": info,
-            "launch_mode": f"stream launches (fixed rule): median of {R} brackets of exactly {K} calls each",
-        })
+        }
         spread = lambda v: {"median": statistics.median(v), "min": min(v), "max": max(v), "n": len(v)}
         line = {
             "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world, "steps": K,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "strong" if by_planes else "weak",
             "vs_baseline": None, "dtype": DTYPE, "data": "synthetic",
-            "config": config,
+            "config": config, "config_detail": detail,
             "votes_per_s": votes_all * jobs * 1e3 / ms_per_step, "votes_per_step": votes_all, "peaks_per_step": n_found,
             "hit_a_evaluations_per_s": n_hits * bn.n_a * jobs * 1e3 / ms_per_step,
             "parity_vs_oracle": "bit-exact" if parity else "MISMATCH",
