@@ -55,7 +55,7 @@ def measured_hbm_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def workload_config(wl, n_hits, n_ev, steps, reps):
+def workload_config(wl, n_hits, n_ev):
     """The `config` block: BOTH arms print exactly this dict (same keys, same values) for the same workload and flags."""
     bn = wl.binning
     m_bytes = 4 * bn.cells * n_ev
@@ -63,14 +63,14 @@ def workload_config(wl, n_hits, n_ev, steps, reps):
             "hits_per_step": int(n_hits), "events_per_step": int(n_ev), "threshold": int(wl.threshold),
             "l2": f"M_H per step ({m_bytes / 1e6:.0f} MB) is larger than the 126 MB L2, and the CUDA arm rotates its output "
                   "matrices, so no step inherits another step's lines",
-            "launch_mode": f"CUDA arm: plain stream launches (fixed rule), median of {reps} brackets of exactly {steps} calls each; "
-                           "reference arm: the CPU oracle as it stands, one thread, the steps timed in one bracket"}
+            "launch_mode": "CUDA arm: plain stream launches (fixed rule), median of the --reps brackets of exactly --steps calls each; "
+                           "reference arm: the CPU oracle as it stands, one thread, the --steps steps timed in one bracket"}
 
 
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
-    def __init__(self, index: int, period_s: float = 0.005):
+    def __init__(self, index: int, period_s: float = 0.001):
         super().__init__(daemon=True)
         self.index, self.period, self.samples, self.reasons, self.stop_flag = index, period_s, [], set(), False
         self.max_mhz = None
@@ -175,7 +175,7 @@ def bench_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": DTYPE, "data": "synthetic",
-        "config": workload_config(wl, batch.n_hits, n_ev, args.steps, args.reps),
+        "config": workload_config(wl, batch.n_hits, n_ev),
         "votes_per_s": votes * args.steps / total,
         "cpu_baseline": {"value": value, "unit": "events/s", "cores": 1, "kind": "oracle",
                          "sample": f"{args.steps} steps of {n_ev} full event(s) of this workload, single thread"},
@@ -286,11 +286,9 @@ def bench_ours(args):
         for k in range(max(args.warmup, 3)):
             step(k)
         stream.synchronize()
-        if sampler is not None:
-            sampler.start()
+        if sampler is not None and not sampler.is_alive():
+            sampler.start()                                           # (keeps sampling until the last timed leg: see below)
         all_ms = [bracket(step, steps) for _ in range(reps)]
-        if sampler is not None:
-            sampler.stop_flag = True
         return statistics.median(all_ms), all_ms
 
     fused_ok = True
@@ -347,6 +345,7 @@ def bench_ours(args):
                 graph_ms = (statistics.median(reps_ms), reps_ms)
         except Exception as err:                                      # capture not supported here: stream launches stand
             print(f"bench.py: CUDA graph capture failed ({err!r}); timing stream launches only", file=sys.stderr)
+    sampler.stop_flag = True                                          # clocks were sampled through every timed leg on the device
     # leave the headline path's outputs in the buffers for the parity check below
     last_k = K - 1
     (step_fused if headline == "fused" else step_split)(last_k)
@@ -565,7 +564,7 @@ def bench_ours(args):
         vote_roof["frac_of_slowest_bound"] = vote_roof["bound_us"] / (ms_per_step * 1e3)
 
         info = B.ht_launch_info(ctx)
-        config = workload_config(wl, n_hits, n_ev, K, R)
+        config = workload_config(wl, n_hits, n_ev)
         detail = {
             "path": ("ht_fill_peaks: one kernel does a0-a5 and stores every M_H cell once" if headline == "fused"
                      else "ht_fill + ht_peaks (two kernels)"),
