@@ -14,9 +14,11 @@
  *
  * Conventions
  *   - Pointers named d_* are DEVICE pointers (on cfg.device), h_* are HOST pointers.  The caller owns every
- *     buffer it passes.  The context's device workspace (the angle tables, a few counters, per-hit scratch of the
- *     classification: 24 bytes per hit of cfg.max_hits, 8 bytes per (event, plane); and, if cfg.host_slots > 0, the
- *     input mirror and host_slots vote matrices of the host calls) is either handed in by the caller
+ *     buffer it passes.  The context's device workspace (the angle tables, a few counters, the scratch of the
+ *     classification: 24 bytes per hit of cfg.max_hits and 8 bytes per (event, plane) for batches, one bucket of 16-byte
+ *     records per plane -- at most 32 MB -- and a 128-byte counter line per plane for single events, a 227 KB block of
+ *     zeros; and, if cfg.host_slots > 0, the input mirror and host_slots vote matrices of the host calls) is either
+ *     handed in by the caller
  *     (ht_query_sizes -> allocate -> ht_create_ex: the library then allocates NOTHING on the device) or allocated by
  *     ht_create itself (convenience form).  With cfg.host_slots > 0 the context also owns pinned HOST staging blocks.
  *   - Layout of a vote matrix (R15): uint32 M[event][itheta][iphi][ia][ib], ib fastest;
@@ -136,9 +138,9 @@ HT_API int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning_or_null, v
  *   d_mh              device, n_events * cells uint32, FULLY OVERWRITTEN: every cell is stored exactly once
  *                     (zero or its count); it need not be cleared beforehand.  4-byte aligned; 16-byte alignment
  *                     (and n_b % 4 == 0) lets the rows leave as bulk (TMA) stores, otherwise plain stores are used.
- * One persistent kernel (cooperative launch, one CTA per SM): the grid classifies every hit once into its
- * (event, theta, phi) plane, then builds tiles of A rows as private shared-memory histograms (a warp owns a row) and
- * stores each tile once with a bulk (TMA) copy: no global atomics on the matrix, no memset pass.
+ * One persistent kernel (one co-resident CTA per SM): the grid classifies every hit once into its (event, theta, phi)
+ * plane, then builds tiles of A rows as private shared-memory histograms (29 warps vote on equal shares of the tile's
+ * hits x rows) and stores each tile once with a bulk (TMA) copy: no global atomics on the matrix, no memset pass.
  * HT_ERR_UNSUPPORTED if one A row (n_b*4 bytes) does not fit a shared-memory slab (two slabs share ~220 KB:
  * n_b > ~27000), if the device cannot launch cooperatively, or if a batch has 2^31 tiles or more: ht_fill_naive.
  */

@@ -161,7 +161,7 @@ WorkspaceLayout workspace_layout(const ht_config *c)
 }
 
 // Tile geometry of the fill kernel for one call: the largest slab (rows of NB cells) such that two slabs, the row
-// tables, the staged hits and -- in mode 1 -- the plane offsets and the uint16 hit index fit the CTA's shared memory.
+// tables and -- in mode 1 -- the plane counts fit the CTA's shared memory.
 struct FillPlan {
     bool ok = false;
     int mode = 0, rows_slab = 0;
