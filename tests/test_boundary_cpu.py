@@ -43,6 +43,41 @@ def test_no_environment_variable_is_read_by_the_library():
     assert C.sizeof(B.ht_tuning) == 64
 
 
+def test_record_layouts_of_the_binding_match_the_header():
+    """The numpy / ctypes records the binding marshals have the sizes and field orders include/ht.h declares."""
+    text = open(os.path.join(ROOT, "include", "ht.h")).read()
+
+    def fields(struct):
+        body = re.search(r"typedef struct %s \{(.*?)\} %s;" % (struct, struct), text, re.S).group(1)
+        body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+        names = []
+        for decl in body.split(";"):
+            decl = decl.strip()
+            if decl:
+                names += [n.strip().split("[")[0] for n in decl.split(None, 1)[1].split(",")]
+        return names
+
+    assert fields("ht_peak") == list(B.PEAK_DTYPE.names) and B.PEAK_DTYPE.itemsize == 12
+    assert fields("ht_track") == list(B.TRACK_DTYPE.names) and B.TRACK_DTYPE.itemsize == 20
+    assert fields("ht_candidate") == list(B.CAND_DTYPE.names) and B.CAND_DTYPE.itemsize == 24
+    assert fields("ht_truth") == list(B.TRUTH_DTYPE.names) and B.TRUTH_DTYPE.itemsize == 24
+    assert fields("ht_match_summary") == list(B.SUMMARY_DTYPE.names) and B.SUMMARY_DTYPE.itemsize == 80
+    assert fields("ht_tuning") == [n for n, _ in B.ht_tuning._fields_]
+    assert fields("ht_config") == [n for n, _ in B.ht_config._fields_]
+
+
+def test_both_bench_arms_print_the_same_config():
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(ROOT, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    wl = WORKLOADS[2]
+    c = bench.workload_config(wl, 5000, 1)
+    assert c["workload"] == "config2:paper_single" and c["bins"] == [4, 16, 1024, 1024] and c["hits_per_step"] == 5000
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert src.count("= workload_config(wl,") + src.count(": workload_config(wl,") == 2      # one call per arm, nothing else builds a `config`
+
+
 def test_no_torch_types_in_the_header():
     text = open(os.path.join(ROOT, "include", "ht.h")).read()
     assert "torch" not in text.replace("torch.cuda.Stream().cuda_stream", "") and "at::" not in text
