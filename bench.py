@@ -233,6 +233,8 @@ def bench_ours(args):
     d_nf = torch.zeros(1, dtype=torch.int32, device=dev)
     T = wl.threshold
     K, R = args.steps, max(args.reps, 1)
+    # device cycles the gate kernel spins per queued call (~15 us each at 2 GHz: more than the host needs to enqueue one)
+    gate_cycles = 0 if args.no_gate or not hasattr(torch.cuda, "_sleep") else 30000
 
     def step_fused(k):                                # a0-a5 in ONE kernel, matrix materialised
         B.ht_fill_peaks(ctx, dx, dy, dz, doff, n_ev, n_hits, mhs[k % n_rot], T, d_out, cap, d_nf, stream)
@@ -271,9 +273,15 @@ def bench_ours(args):
         return ms
 
     def bracket(step, steps):
-        """Exactly `steps` calls between barrier + synchronize; CUDA events on the launch stream; max over ranks."""
+        """Exactly `steps` calls between barrier + synchronize; CUDA events on the launch stream; max over ranks.
+        The stream first gets a short spin kernel, so that the calls are already queued when the first event fires: the
+        bracket then times the device executing `steps` calls back to back, not the host enqueuing the first of them
+        (~10 us after an idle stream, which a 20-step bracket would otherwise book as 0.5 us per step)."""
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if gate_cycles:
+            with torch.cuda.stream(stream):
+                torch.cuda._sleep(gate_cycles * min(steps, 64))
         e0.record(stream)
         for k in range(steps):
             step(k)
@@ -569,6 +577,9 @@ def bench_ours(args):
             "path": ("ht_fill_peaks: one kernel does a0-a5 and stores every M_H cell once" if headline == "fused"
                      else "ht_fill + ht_peaks (two kernels)"),
             "rotated_output_matrices": n_rot,
+            "bracket_gate": ("a spin kernel of ~15 us per queued call (at most 64) runs ahead of the first event of every bracket, so the "
+                             "calls are queued when timing starts (device time of K back-to-back calls)" if gate_cycles
+                             else "none: the host's enqueue latency of the first call is inside the bracket"),
             "launch": info,
         }
         spread = lambda v: {"median": statistics.median(v), "min": min(v), "max": max(v), "n": len(v)}
@@ -627,6 +638,7 @@ def main():
                     help="headline path: ht_fill_peaks (one kernel) or ht_fill + ht_peaks")
     ap.add_argument("--rotate", type=int, default=4, help="number of output matrices rotated between steps")
     ap.add_argument("--no-graph", action="store_true", help="skip the CUDA graph replay leg")
+    ap.add_argument("--no-gate", action="store_true", help="no spin kernel ahead of a bracket (the host's first enqueue is timed too)")
     ap.add_argument("--no-cpu-all-cores", action="store_true", help="skip the all-cores CPU line")
     ap.add_argument("--split", choices=["events", "planes"], default="events",
                     help="N > 1: every rank its own events (weak scaling, default) or the same events split by plane")
