@@ -111,7 +111,10 @@ typedef struct ht_tuning {
     int32_t peaks_ctas_per_sm;         /* > 0: cap of the peak scan's resident CTAs per SM */
     int32_t fill_store_warps;          /* 1: one store warp queues every tile store; 2: one store warp per slab (0: chosen
                                           from the hits per plane of the call) */
-    int32_t reserved[8];               /* must be zero */
+    int32_t fill_early_cap;            /* single events of <= 32768 hits: every CTA finds the hits of its first tile's plane
+                                          itself and votes while the grid still classifies ("early tiles").  > 0: records of
+                                          that list in shared memory; 0: three times the average plane + 32; -1: no early tiles */
+    int32_t reserved[7];               /* must be zero */
 } ht_tuning;
 
 /* Sizes implied by a configuration: bytes of one event's matrix, and bytes of the context's device workspace
@@ -162,6 +165,17 @@ HT_API int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const 
                          const int32_t *d_event_offsets, int32_t n_events, int32_t n_hits_total,
                          uint32_t *d_mh_or_null, uint32_t threshold, ht_peak *d_out, uint32_t capacity,
                          uint32_t *d_n_found, void *cuda_stream);
+
+/* A promise about the INPUTS of this context's following ht_fill / ht_fill_peaks calls (on != 0; revoked with 0; off by
+ * default).  The caller states that, for each such call, every write to d_x, d_y, d_z and d_event_offsets had COMPLETED
+ * before the call was made (a batch of events staged in device memory and synchronized once, then one call per event:
+ * the paper's use), or had been enqueued on the call's stream before the previous call of this
+ * context; and that nothing enqueued later writes them before the call has run.  The kernel then reads the hits as soon
+ * as its thread blocks are resident -- while the previous kernel of the stream is still draining (dependent launch) --
+ * instead of after that kernel has completed; it still writes nothing before.  Results are the same; a single-event
+ * call in a stream of calls saves the ~3 us its first tile's hits take to find.  With the promise broken the kernel may
+ * read hits that are not yet written.  (Defines no step of the method.) */
+HT_API int ht_promise_stable_inputs(ht_ctx *ctx, int32_t on);
 
 /* The paper's own design (cudaMemset, one block per hit, threads over A, global atomicAdd),
  * same arguments and result as ht_fill, any binning.  Kept as the prior-art comparison and for shapes ht_fill

@@ -28,7 +28,7 @@ SUMMARY_DTYPE = np.dtype([("n_cand", np.int64), ("n_truth", np.int64), ("n_match
                           ("n_found", np.int64), ("n_duplicate", np.int64), ("sum_drho", np.float64),
                           ("sum_drho2", np.float64), ("sum_dphi", np.float64), ("sum_dphi2", np.float64)])   # == ht_match_summary
 
-EXPORTS = ("ht_query_sizes", "ht_create", "ht_create_ex", "ht_fill", "ht_fill_peaks", "ht_fill_naive", "ht_peaks", "ht_tracks",
+EXPORTS = ("ht_query_sizes", "ht_create", "ht_create_ex", "ht_fill", "ht_fill_peaks", "ht_promise_stable_inputs", "ht_fill_naive", "ht_peaks", "ht_tracks",
            "ht_merge_scratch_bytes", "ht_merge_ridges", "ht_match_truth",
            "ht_run_host", "ht_run_host_events", "ht_submit_host", "ht_wait_host", "ht_destroy", "ht_strerror")                  # include/ht.h
 DIAG_EXPORTS = ("ht_tables_host", "ht_kernel_launches", "ht_launch_info", "ht_selftest_division", "ht_diag_memset",
@@ -64,7 +64,7 @@ class ht_tuning(C.Structure):
     _fields_ = [("fill_batch_classification", C.c_int32), ("fill_slab_kb", C.c_int32),
                 ("fill_plain_stores", C.c_int32), ("cooperative_launch", C.c_int32),
                 ("host_copy_input", C.c_int32), ("peaks_unroll", C.c_int32), ("peaks_ctas_per_sm", C.c_int32),
-                ("fill_store_warps", C.c_int32), ("reserved", C.c_int32 * 8)]
+                ("fill_store_warps", C.c_int32), ("fill_early_cap", C.c_int32), ("reserved", C.c_int32 * 7)]
 
 
 class HtError(RuntimeError):
@@ -110,6 +110,8 @@ def load() -> C.CDLL:
     lib.ht_fill_peaks.restype = C.c_int
     lib.ht_fill_peaks.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, u32, vp, u32, vp, vp]
     lib.ht_peaks.restype = C.c_int
+    lib.ht_promise_stable_inputs.restype = C.c_int
+    lib.ht_promise_stable_inputs.argtypes = [vp, i32]
     lib.ht_peaks.argtypes = [vp, vp, i32, u32, vp, u32, vp, vp]
     lib.ht_tracks.restype = C.c_int
     lib.ht_tracks.argtypes = [vp, vp, u32, vp, vp]
@@ -209,6 +211,11 @@ def ht_fill_peaks(ctx, d_x, d_y, d_z, d_event_offsets, n_events: int, n_hits_tot
     _check(load().ht_fill_peaks(ctx, _ptr(d_x), _ptr(d_y), _ptr(d_z), _ptr(d_event_offsets), n_events, n_hits_total,
                                 _ptr(d_mh), threshold, _ptr(d_out), capacity, _ptr(d_n_found), _stream(stream)),
            "ht_fill_peaks")
+
+
+def ht_promise_stable_inputs(ctx, on: bool = True) -> None:
+    """The inputs of the following ht_fill / ht_fill_peaks calls are final before each call is made (include/ht.h)."""
+    _check(load().ht_promise_stable_inputs(ctx, 1 if on else 0), "ht_promise_stable_inputs")
 
 
 def ht_fill_naive(ctx, d_x, d_y, d_z, d_event_offsets, n_events: int, n_hits_total: int, d_mh, stream=None) -> None:

@@ -165,6 +165,7 @@ WorkspaceLayout workspace_layout(const ht_config *c)
 struct FillPlan {
     bool ok = false;
     int mode = 0, rows_slab = 0;
+    int early_cap = 0;                 // records of the early tiles' list in shared memory (0: no early tiles)
     uint32_t slab_words = 0;
     size_t smem = 0;
 };
@@ -185,6 +186,8 @@ struct ht_ctx {
     ht_tuning tun;
     ht::Geom geom;
     float two_a_absmax = 0.0f;             // max |2 * A_c| over the A rows
+    bool stable_inputs = false;            // ht_promise_stable_inputs
+    bool tables_monotone = false;          // T non-increasing, P non-decreasing, no NaN: a bin of the bisection is an interval (early tiles)
     int sm_count = 0;
     int max_smem_optin = 0;
     // device workspace
@@ -222,12 +225,11 @@ struct ht_ctx {
 
 namespace {
 
-size_t fill_smem_bytes(const ht_config &c, long long rows, int mode, long long n_hits)
+size_t fill_smem_bytes(const ht_config &c, long long rows, int mode, long long early_cap)
 {
     const size_t slab = align_up((size_t)rows * (size_t)c.n_b * 4u, 16);
     size_t b = 2u * slab + 8u * 4u * (size_t)((rows + 7) & ~3ll);     // two slabs, two_a[8 ring entries][rows + 4, rounded up to 4]
-    if (mode == 1) b += 4u * (size_t)c.n_theta * (size_t)c.n_phi;            // hits per plane
-    (void)n_hits;
+    if (mode == 1) b += 4u * align_up((size_t)c.n_theta * (size_t)c.n_phi, 4) + 16u * (size_t)early_cap;   // hits per plane; early list
     return align_up(b, 16);
 }
 
@@ -295,7 +297,7 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
         for (int32_t r : tun.reserved)
             if (r != 0) return HT_ERR_INVALID_ARG;
         if (tun.peaks_unroll != 0 && tun.peaks_unroll != 2 && tun.peaks_unroll != 4 && tun.peaks_unroll != 8) return HT_ERR_INVALID_ARG;
-        if (tun.fill_slab_kb < 0 || tun.peaks_ctas_per_sm < 0 || tun.fill_store_warps < 0 || tun.fill_store_warps > 2) return HT_ERR_INVALID_ARG;
+        if (tun.fill_slab_kb < 0 || tun.peaks_ctas_per_sm < 0 || tun.fill_store_warps < 0 || tun.fill_store_warps > 2 || tun.fill_early_cap < -1) return HT_ERR_INVALID_ARG;
     }
     const WorkspaceLayout lay = workspace_layout(cfg);
     if (d_workspace && (workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0)) return HT_ERR_INVALID_ARG;
@@ -325,6 +327,9 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
         build_tables(cfg, two_a.data(), tth.data(), pph.data(), d_ab);
         ctx->two_a_absmax = std::max(std::fabs(two_a.front()), std::fabs(two_a.back()));
     }
+    ctx->tables_monotone = true;
+    for (size_t k = 0; k + 1 < tth.size(); ++k) ctx->tables_monotone = ctx->tables_monotone && tth[k] >= tth[k + 1];
+    for (size_t k = 0; k + 1 < pph.size(); ++k) ctx->tables_monotone = ctx->tables_monotone && pph[k] <= pph[k + 1];
 
     cudaError_t e;
     auto fail = [&](int code) { ht_destroy(ctx); return code; };
@@ -455,16 +460,26 @@ FillPlan compute_fill_plan(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, 
     // without the fused peak search the kernel is purely store-bound and measured fastest with slabs of <= 96 KB
     // (config 2, B200: 51.5 us at 96 KB, 53.4 at 100 KB, 59.4 at 104 KB); with it, the largest slab wins (fewer halo rows)
     const int slab_kb = tun.fill_slab_kb > 0 ? tun.fill_slab_kb : (peaks ? 0 : 96);
+    // early tiles (mode 1, not too many hits): a CTA keeps the records of ONE plane's hits in shared memory -- room for
+    // three times the average plane (the planes of the outer theta bins hold twice the average), at most every hit; a
+    // plane with more falls back to the buckets
+    auto early_cap_for = [&](int md) -> long long {
+        if (md != 1 || tun.fill_early_cap < 0 || n_hits < 1 || n_hits > ht::kEarlyMaxHits || !ctx->tables_monotone) return 0;
+        long long cap = tun.fill_early_cap > 0 ? tun.fill_early_cap : 3 * ((n_hits + planes - 1) / planes) + 32;
+        if (cap > n_hits) cap = n_hits;
+        return (long long)align_up((size_t)cap, 4);
+    };
     auto rows_for = [&](int md) -> long long {
+        const long long ecap = early_cap_for(md);
         const size_t budget = budget_all;
         long long rows = c.n_a;
         if (slab_kb > 0 && rows > (long long)((size_t)slab_kb * 1024u / row_bytes)) rows = (long long)((size_t)slab_kb * 1024u / row_bytes);
         if (rows < 1) rows = 1;
-        if (fill_smem_bytes(c, rows, md, n_hits) > budget) {                  // largest rows that fit (bisection)
+        if (fill_smem_bytes(c, rows, md, ecap) > budget) {                  // largest rows that fit (bisection)
             long long lo = 0, hi = rows;
             while (hi - lo > 1) {
                 const long long mid = (lo + hi) / 2;
-                if (fill_smem_bytes(c, mid, md, n_hits) <= budget) lo = mid; else hi = mid;
+                if (fill_smem_bytes(c, mid, md, ecap) <= budget) lo = mid; else hi = mid;
             }
             rows = lo;
         }
@@ -477,7 +492,8 @@ FillPlan compute_fill_plan(const ht_ctx *ctx, int32_t n_events, int32_t n_hits, 
             pl.mode = mode;
             pl.rows_slab = (int)rows;
             pl.slab_words = (uint32_t)(align_up((size_t)rows * row_bytes, 16) / 4u);
-            pl.smem = fill_smem_bytes(c, rows, mode, n_hits);
+            pl.early_cap = (int)early_cap_for(mode);
+            pl.smem = fill_smem_bytes(c, rows, mode, pl.early_cap);
             return pl;
         }
         if (mode == 0) return pl;                                              // one row does not fit: ht_fill_naive only
@@ -498,10 +514,12 @@ const FillPlan &plan_fill(ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool pe
 // The fill kernel (prologue a0 + tiles a1-a3), with (PEAKS: + a4-a5) or without the fused peak search.
 // early_inputs: the hit arrays are known not to be written by device work enqueued before this call (the context's own
 // pinned staging blocks), so the kernel may read them before the previous kernel of the stream has completed.
+enum { kInputsPlain = 0, kInputsStable = 1, kInputsHostMapped = 2 };
 int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off, int32_t n_events,
                 int32_t n_hits_total, uint32_t *d_mh, bool peaks, uint32_t threshold, ht_peak *d_out, uint32_t capacity,
-                uint32_t *d_n_found, cudaStream_t st, bool early_inputs, uint32_t *d_done_flag = nullptr, uint32_t done_value = 0u)
+                uint32_t *d_n_found, cudaStream_t st, int input_kind, uint32_t *d_done_flag = nullptr, uint32_t done_value = 0u)
 {
+    const bool early_inputs = input_kind != kInputsPlain;
     const ht::Geom &g = ctx->geom;
     const FillPlan &pl = plan_fill(ctx, n_events, n_hits_total, peaks);
     if (!pl.ok) return HT_ERR_UNSUPPORTED;
@@ -512,6 +530,8 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.counts = ctx->d_counts; a.counts1 = ctx->d_counts1; a.zeros = ctx->d_zeros; a.bucket_start = ctx->d_bucket_start; a.h_plane = ctx->d_hplane; a.h_rel = ctx->d_hrel;
     a.bx = pl.mode == 1 ? ctx->d_buckets : ctx->d_bx;
     a.bucket_cap = (int)align_up((size_t)n_hits_total, 4);
+    // early tiles: not when the hits sit in pinned host memory (every CTA reads all of them)
+    a.early_cap = input_kind == kInputsHostMapped ? 0 : pl.early_cap;
     a.two_a_absmax = ctx->two_a_absmax;
     // one queue of tile stores while the store is the slow part; a store warp per slab when the votes are (more than
     // ~150 hits per (event, plane): config 4)
@@ -557,6 +577,10 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     // so the launch can be captured into a CUDA graph and replayed
     a.tile_counter = ctx->d_counters + 6;
     a.bar_count = ctx->d_counters + 5;
+    // the first two tiles of a CTA: neighbours (2c, 2c+1: mostly one plane, one early list) when every CTA has two
+    a.pair_tiles = n_tiles >= 2ull * grid ? 1 : 0;
+    // one tile per CTA and an early list that holds every hit: nothing needs the buckets
+    a.skip_classify = (a.early_cap > 0 && n_tiles <= grid && n_hits_total <= a.early_cap) ? 1 : 0;
     const void *fn = peaks ? reinterpret_cast<const void *>(ht::fill_tiles_kernel<true>)
                            : reinterpret_cast<const void *>(ht::fill_tiles_kernel<false>);
     void *params[] = {&a};
@@ -595,7 +619,7 @@ int ht_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, c
     if (rc != HT_OK || n_events == 0) return rc;
     DeviceGuard guard(ctx->cfg.device);
     return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh, false, 0u, nullptr, 0u, nullptr,
-                       static_cast<cudaStream_t>(cuda_stream), false);
+                       static_cast<cudaStream_t>(cuda_stream), ctx->stable_inputs ? kInputsStable : kInputsPlain);
 }
 
 int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
@@ -612,7 +636,14 @@ int ht_fill_peaks(ht_ctx *ctx, const float *d_x, const float *d_y, const float *
         return HT_OK;
     }
     return launch_fill(ctx, d_x, d_y, d_z, d_event_offsets, n_events, n_hits_total, d_mh_or_null, true, threshold, d_out, capacity,
-                       d_n_found, st, false);
+                       d_n_found, st, ctx->stable_inputs ? kInputsStable : kInputsPlain);
+}
+
+int ht_promise_stable_inputs(ht_ctx *ctx, int32_t on)
+{
+    if (!ctx) return HT_ERR_INVALID_ARG;
+    ctx->stable_inputs = on != 0;
+    return HT_OK;
 }
 
 int ht_fill_naive(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_event_offsets,
@@ -709,8 +740,8 @@ int enqueue_group(ht_ctx *ctx, HostSlot &sl, const unsigned char *in_base, const
     ht_peak *d_list = reinterpret_cast<ht_peak *>(sl.d_res + kResHeader);
     // the kernel itself tells the host when the results are in the mapped block (second word of the header)
     sl.flagged = flag;
-    int rc = launch_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, true, threshold, d_list, room, d_count, st, early_inputs,
-                         flag ? d_count + 1 : nullptr, sl.seq);
+    int rc = launch_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, true, threshold, d_list, room, d_count, st,
+                         early_inputs ? kInputsHostMapped : kInputsPlain, flag ? d_count + 1 : nullptr, sl.seq);
     if (rc == HT_ERR_UNSUPPORTED) {
         sl.flagged = false;
         rc = ht_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, st);
@@ -1072,11 +1103,11 @@ int ht_diag_vote_rates(int32_t device, int32_t iters, double *h_rates, uint64_t 
 // build-time instrumentation only: copy (and clear) the per-CTA phase counters of the fill kernel
 __attribute__((visibility("default"))) int ht_prof_read(uint64_t *h_out, int32_t n_words, int32_t reset)
 {
-    if (!h_out || n_words < 0 || n_words > 256 * 16) return HT_ERR_INVALID_ARG;
+    if (!h_out || n_words < 0 || n_words > 256 * 32) return HT_ERR_INVALID_ARG;
     HT_CUDA(cudaDeviceSynchronize());
     HT_CUDA(cudaMemcpyFromSymbol(h_out, ht::g_prof, sizeof(uint64_t) * (size_t)n_words));
     if (reset) {
-        static const unsigned long long zeros[256 * 16] = {};
+        static const unsigned long long zeros[256 * 32] = {};
         HT_CUDA(cudaMemcpyToSymbol(ht::g_prof, zeros, sizeof zeros));
     }
     return HT_OK;

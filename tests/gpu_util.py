@@ -24,6 +24,8 @@ class GpuHough:
         self.cfg = B.ht_config.from_binning(binning, max_events=max_events, max_hits=max(1, max_hits), device=0,
                                             host_slots=host_slots, host_peak_capacity=host_peak_capacity)
         self.dev = torch.device("cuda:0")
+        tuning = dict(tuning) if tuning else None
+        stable = bool(tuning.pop("stable_inputs", 0)) if tuning else False      # (not a tuning field: ht_promise_stable_inputs)
         self.tuning = B.ht_tuning(**tuning) if tuning else None
         self.workspace = None
         if own_workspace:
@@ -35,6 +37,8 @@ class GpuHough:
             self.ctx = B.ht_create_ex(self.cfg, self.tuning)
         else:
             self.ctx = B.ht_create(self.cfg)
+        if stable:
+            B.ht_promise_stable_inputs(self.ctx, True)
 
     def close(self):
         B.ht_destroy(self.ctx)

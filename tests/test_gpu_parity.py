@@ -3,6 +3,8 @@
 Bar (BASELINE.json north_star): the vote matrix and the sorted peak list are BIT-EXACT.  Integer work throughout;
 the floating point that decides bin indices is IEEE binary32 on both sides (SPEC.md section 0).
 """
+import math
+
 import numpy as np
 import pytest
 import torch
@@ -322,7 +324,8 @@ def test_fused_kernel_list_truncation():
             assert n2 == len(want) and len(got2) == len(want) - 1 and got2 <= full
 
 
-@pytest.mark.parametrize("tuning", [None, {"fill_batch_classification": 1}, {"cooperative_launch": 1}, {"fill_store_warps": 2}])
+@pytest.mark.parametrize("tuning", [None, {"fill_batch_classification": 1}, {"cooperative_launch": 1}, {"fill_store_warps": 2},
+                                    {"fill_early_cap": -1}, {"stable_inputs": 1}, {"fill_early_cap": 8, "stable_inputs": 1}])
 def test_repeated_launches_give_the_same_bits(tuning):
     """No timing-dependent result: 3000 back-to-back fused launches per variant (hand-rolled grid barrier, named-barrier
     pipeline, TMA proxy fence, dependent launches overlapping their predecessor's tail), matrix and peak set compared on
@@ -469,6 +472,11 @@ def test_error_codes_on_device_calls():
                                     {"cooperative_launch": 1},           # cudaLaunchCooperativeKernel instead of the dependent launch
                                     {"fill_store_warps": 1}, {"fill_store_warps": 2},      # one queue of tile stores / a store warp per slab
                                     {"fill_store_warps": 2, "fill_slab_kb": 8, "fill_batch_classification": 1},
+                                    {"fill_early_cap": -1},              # no early tiles: every tile from the grid's buckets
+                                    {"fill_early_cap": 8},               # early list too small for most planes: falls back per CTA
+                                    {"fill_early_cap": 8, "fill_store_warps": 2, "fill_slab_kb": 8},
+                                    {"stable_inputs": 1},                # ht_promise_stable_inputs: hits read before the previous kernel completes
+                                    {"stable_inputs": 1, "fill_early_cap": -1}, {"stable_inputs": 1, "fill_slab_kb": 8},
                                     {"peaks_unroll": 4}, {"peaks_unroll": 8, "peaks_ctas_per_sm": 2}])
 def test_fill_kernel_variants_are_bit_exact(tuning):
     """The switches of ht_tuning (read once by ht_create_ex) change how the work is organised, never the result."""
@@ -478,6 +486,45 @@ def test_fill_kernel_variants_are_bit_exact(tuning):
     assert _check_batch(bn, one, wl.threshold, tuning=tuning) > 0
     three = generate_batch(WORKLOADS[3], n_events=3)
     assert _check_batch(bn, three, wl.threshold, tuning=tuning, own_workspace=True) > 0
+
+
+def test_hits_on_the_edges_of_the_angle_bins():
+    """Early tiles decide "is this hit in my plane" by comparing q and p with the plane's two table entries instead of
+    bisecting the tables (and a coarse test with approximate reciprocals decides which hits get that far): hits whose q
+    or p IS a table entry, or one ulp beside it, on every edge of both tables, with and without early tiles."""
+    bn = Binning(4, 16, 128, 256)
+    cfg = B.ht_config.from_binning(bn, max_events=1, max_hits=1, device=0)
+    _, tth, pph, _, _ = B.ht_tables_host(cfg)
+    xs, ys, zs = [], [], []
+    f32 = np.float32
+    ulps = lambda v: [np.nextafter(f32(v), f32(-np.inf)), f32(v), np.nextafter(f32(v), f32(np.inf))]
+    # q = z / sqrt(x^2 + y^2): with r = 64 (a power of two, r^2 exact) q = z / 64 is exact, so z = 64 * T[k] puts q on T[k]
+    for k, t in enumerate(tth):
+        if not np.isfinite(t):
+            continue
+        for q in ulps(t):
+            for phi in (0.3, 2.0, 4.1, 5.5):
+                x, y = f32(64.0 * math.cos(phi)), f32(64.0 * math.sin(phi))
+                r = math.sqrt(float(x) ** 2 + float(y) ** 2)
+                xs.append(x); ys.append(y); zs.append(f32(float(q) * r))
+    # p = 1 - x / (|x| + |y|) (y >= 0) or 3 + x / (|x| + |y|): x = d * (1 - P[k]) with d = |x| + |y| = 64
+    for k, pe in enumerate(pph):
+        for pv in ulps(pe):
+            pv = float(pv)
+            u = 1.0 - pv if pv <= 2.0 else pv - 3.0                  # x / d
+            if abs(u) > 1.0:
+                continue
+            x = f32(64.0 * u)
+            y = f32((64.0 - abs(float(x))) * (1.0 if pv <= 2.0 else -1.0))
+            for z in (-50.0, 3.0, 80.0):
+                xs.append(x); ys.append(y); zs.append(f32(z))
+    rng = np.random.default_rng(5)
+    reps = 6                                                            # several votes per cell, so that peaks exist
+    x = np.tile(np.asarray(xs, f32), reps); y = np.tile(np.asarray(ys, f32), reps); z = np.tile(np.asarray(zs, f32), reps)
+    perm = rng.permutation(len(x))
+    batch = batch_from_arrays([np.stack([x[perm], y[perm], z[perm]], axis=1)])
+    for tuning in (None, {"fill_early_cap": -1}, {"stable_inputs": 1}):
+        assert _check_batch(bn, batch, 3, tuning=tuning) >= 0
 
 
 def test_caller_owned_workspace_and_bad_tuning():
