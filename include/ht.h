@@ -103,10 +103,14 @@ typedef struct ht_tuning {
     int32_t fill_plain_stores;         /* 1: tiles leave with plain stores instead of bulk (TMA) stores */
     int32_t cooperative_launch;        /* 1: cudaLaunchCooperativeKernel (0: ordinary launch, programmatic dependent
                                           launch: the next call's prologue overlaps this call's tail) */
-    int32_t host_copy_input;           /* 0: the kernel of a single host event reads the hits straight from the pinned block
-                                          (zero-copy over PCIe, coalesced; no copy call and no event between two kernels of
-                                          the stream, so consecutive events keep their dependent launch: 52 us per pipelined
-                                          event); 1: one asynchronous copy per event on a second stream (56 us) */
+    int32_t host_copy_input;           /* how the hits of a single host event (ht_submit_host) reach the kernel.  1: one
+                                          asynchronous copy into device memory on a second stream, which also writes the
+                                          submission's number behind the hits; the kernel waits for that word itself, so no
+                                          event stands between two kernels of the compute stream and consecutive events keep
+                                          their dependent launch.  2: the kernel reads them straight from the pinned block
+                                          (zero-copy over PCIe, coalesced).  0: 1 when the call uses early tiles (which read
+                                          every hit in every thread block), else 2.  (47.2 / 48.2 us per pipelined event of
+                                          5000 hits, 71.3 / 69.9 us at 20000) */
     int32_t peaks_unroll;              /* 2, 4 or 8 independent 16-byte loads per thread of the peak scan (0: 2) */
     int32_t peaks_ctas_per_sm;         /* > 0: cap of the peak scan's resident CTAs per SM */
     int32_t fill_store_warps;          /* 1: one store warp queues every tile store; 2: one store warp per slab (0: chosen

@@ -124,6 +124,8 @@ constexpr size_t kResHeader = 16;      // result block: [uint32 n_found, pad to 
 
 // Layout of the context's device workspace (one contiguous block: caller-owned or allocated by ht_create) and sizes of
 // the pinned host staging blocks.  Offsets are multiples of 256.
+constexpr size_t kInTrailer = 16;     // last bytes of a slot's input block: the number of the submission whose hits the block holds
+
 struct WorkspaceLayout {
     size_t tables, counters, hits, buckets, bucket_start, counts, counts1, zeros, in_dev, mh;      // offsets
     size_t hits_part;             // bytes of one of the 6 per-hit arrays
@@ -151,7 +153,7 @@ WorkspaceLayout workspace_layout(const ht_config *c)
     w.zeros = take(kZeroBytes);                // source of the TMA's zero fill of a slab (at most the CTA's shared memory)
     if (c->host_slots > 0) {
         w.in_block = align_up(align_up(sizeof(int32_t) * ((size_t)c->max_events + 1), 16) +
-                              3 * align_up(sizeof(float) * (size_t)c->max_hits, 16), 256);
+                              3 * align_up(sizeof(float) * (size_t)c->max_hits, 16) + kInTrailer, 256);
         w.res_block = align_up(kResHeader + sizeof(ht_peak) * (size_t)c->host_peak_capacity, 256);
         w.in_dev = take(w.in_block * (size_t)c->host_slots);
         w.mh = take(cells * sizeof(uint32_t) * (size_t)c->host_slots);
@@ -297,7 +299,8 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
         for (int32_t r : tun.reserved)
             if (r != 0) return HT_ERR_INVALID_ARG;
         if (tun.peaks_unroll != 0 && tun.peaks_unroll != 2 && tun.peaks_unroll != 4 && tun.peaks_unroll != 8) return HT_ERR_INVALID_ARG;
-        if (tun.fill_slab_kb < 0 || tun.peaks_ctas_per_sm < 0 || tun.fill_store_warps < 0 || tun.fill_store_warps > 2 || tun.fill_early_cap < -1) return HT_ERR_INVALID_ARG;
+        if (tun.fill_slab_kb < 0 || tun.peaks_ctas_per_sm < 0 || tun.fill_store_warps < 0 || tun.fill_store_warps > 2 || tun.fill_early_cap < -1 ||
+            tun.host_copy_input < 0 || tun.host_copy_input > 2) return HT_ERR_INVALID_ARG;
     }
     const WorkspaceLayout lay = workspace_layout(cfg);
     if (d_workspace && (workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) != 0)) return HT_ERR_INVALID_ARG;
@@ -376,6 +379,9 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
         if ((e = cudaHostAlloc((void **)&ctx->h_res_all, lay.res_block * ns, cudaHostAllocMapped)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaHostAlloc(result)"));
         std::memset(ctx->h_res_all, 0, lay.res_block * ns);          // (the completion word of a slot starts at 0, its first submission is number 1)
+        std::memset(ctx->h_in_all, 0, lay.in_block * ns);
+        if ((e = cudaMemset(ws + lay.in_dev, 0, lay.in_block * ns)) != cudaSuccess)      // (so does the "copied" word of its device block)
+            return fail(cuda_fail(e, "cudaMemset(input blocks)"));
         unsigned char *in_map = nullptr, *res_map = nullptr;
         if ((e = cudaHostGetDevicePointer((void **)&in_map, ctx->h_in_all, 0)) != cudaSuccess ||
             (e = cudaHostGetDevicePointer((void **)&res_map, ctx->h_res_all, 0)) != cudaSuccess)
@@ -517,7 +523,8 @@ const FillPlan &plan_fill(ht_ctx *ctx, int32_t n_events, int32_t n_hits, bool pe
 enum { kInputsPlain = 0, kInputsStable = 1, kInputsHostMapped = 2 };
 int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off, int32_t n_events,
                 int32_t n_hits_total, uint32_t *d_mh, bool peaks, uint32_t threshold, ht_peak *d_out, uint32_t capacity,
-                uint32_t *d_n_found, cudaStream_t st, int input_kind, uint32_t *d_done_flag = nullptr, uint32_t done_value = 0u)
+                uint32_t *d_n_found, cudaStream_t st, int input_kind, uint32_t *d_done_flag = nullptr, uint32_t done_value = 0u,
+                const uint32_t *d_ready_flag = nullptr)
 {
     const bool early_inputs = input_kind != kInputsPlain;
     const ht::Geom &g = ctx->geom;
@@ -561,6 +568,7 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.early_inputs = early_inputs ? 1 : 0;
     a.done_flag = d_done_flag;
     a.done_value = done_value;
+    a.ready_flag = d_ready_flag;        // (its value: done_value, the number of the submission)
     a.threshold = threshold;
     static_assert(sizeof(ht::PeakOut) == sizeof(ht_peak), "peak record layout");
     a.out = reinterpret_cast<ht::PeakOut *>(d_out);
@@ -729,7 +737,8 @@ InBlock in_block(const ht_ctx *ctx, int32_t n_hits)
 // One group of events (at most host_slots, all in the input block of slot `s`, matrices from `mh_slot` on) through the
 // fused kernel (or the two-call path for shapes it refuses), peak list and count into slot s's mapped result block.
 int enqueue_group(ht_ctx *ctx, HostSlot &sl, const unsigned char *in_base, const InBlock &ib, int32_t hit_base, int32_t ne,
-                  int32_t nh, uint32_t *d_mh, uint32_t threshold, uint32_t room, bool early_inputs, bool flag = false)
+                  int32_t nh, uint32_t *d_mh, uint32_t threshold, uint32_t room, int input_kind, bool flag = false,
+                  const uint32_t *d_ready_flag = nullptr)
 {
     cudaStream_t st = ctx->host_stream;
     const float *d_x = reinterpret_cast<const float *>(in_base + ib.o_x) + hit_base;
@@ -741,9 +750,13 @@ int enqueue_group(ht_ctx *ctx, HostSlot &sl, const unsigned char *in_base, const
     // the kernel itself tells the host when the results are in the mapped block (second word of the header)
     sl.flagged = flag;
     int rc = launch_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, true, threshold, d_list, room, d_count, st,
-                         early_inputs ? kInputsHostMapped : kInputsPlain, flag ? d_count + 1 : nullptr, sl.seq);
+                         input_kind, flag ? d_count + 1 : nullptr, sl.seq, d_ready_flag);
     if (rc == HT_ERR_UNSUPPORTED) {
         sl.flagged = false;
+        if (d_ready_flag) {             // (the other kernels do not look at the copy's word: order the streams instead)
+            HT_CUDA(cudaEventRecord(sl.copied, ctx->copy_stream));
+            HT_CUDA(cudaStreamWaitEvent(st, sl.copied, 0));
+        }
         rc = ht_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, st);
         if (rc == HT_ERR_UNSUPPORTED) rc = ht_fill_naive(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, st);
         if (rc != HT_OK) return rc;
@@ -779,17 +792,29 @@ int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y
     // One event whose hits the grid reads exactly once (mode 1): straight from the pinned block (zero-copy over PCIe);
     // otherwise one packed copy on the copy stream, which overlaps the kernel of the previous event.
     const FillPlan &pl = plan_fill(ctx, 1, n_hits, true);
-    const bool zero_copy = !ctx->tun.host_copy_input && pl.ok && pl.mode == 1;
+    // (early tiles -- every CTA reads all the hits -- want them in device memory: copy when the plan has them)
+    const bool want_copy = ctx->tun.host_copy_input == 1 || (ctx->tun.host_copy_input == 0 && pl.early_cap > 0);
+    const bool zero_copy = !want_copy && pl.ok && pl.mode == 1;
     const unsigned char *in_base = sl.d_in_mapped;
-    if (!zero_copy) {
-        HT_CUDA(cudaMemcpyAsync(sl.d_in, sl.h_in, ib.bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
-        HT_CUDA(cudaEventRecord(sl.copied, ctx->copy_stream));
-        HT_CUDA(cudaStreamWaitEvent(ctx->host_stream, sl.copied, 0));
-        in_base = sl.d_in;
-    }
     uint32_t *d_mh = ctx->d_hmh + (size_t)slot * (size_t)ctx->geom.cells;
     ++sl.seq;
-    const int rc = enqueue_group(ctx, sl, in_base, ib, 0, 1, n_hits, d_mh, threshold, ctx->cfg.host_peak_capacity, true, true);
+    const uint32_t *d_ready = nullptr;
+    if (!zero_copy) {
+        // Two copies on the copy stream: the block, then the number of this submission into the block's last word.  The
+        // kernel waits for that word itself (its first instruction after it is resident), so nothing stands between two
+        // kernels of the compute stream -- no event, no stream wait: consecutive events keep their dependent launch --
+        // and the copy, enqueued while earlier events are still being computed, is long done when the kernel looks.
+        const size_t o_seq = ctx->lay.in_block - kInTrailer;
+        *reinterpret_cast<uint32_t *>(sl.h_in + o_seq) = sl.seq;
+        HT_CUDA(cudaMemcpyAsync(sl.d_in, sl.h_in, ib.bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+        HT_CUDA(cudaMemcpyAsync(sl.d_in + o_seq, sl.h_in + o_seq, sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->copy_stream));
+        in_base = sl.d_in;
+        d_ready = reinterpret_cast<const uint32_t *>(sl.d_in + o_seq);
+    }
+    // (the slot's blocks are the library's own: final before the kernel reads them -- host-mapped, or announced by the
+    // copy stream)
+    const int rc = enqueue_group(ctx, sl, in_base, ib, 0, 1, n_hits, d_mh, threshold, ctx->cfg.host_peak_capacity,
+                                 zero_copy ? kInputsHostMapped : kInputsStable, true, d_ready);
     if (rc != HT_OK) return rc;
     // (no event between two kernels of the stream when the kernel signals its own completion: an event record there
     // would undo the dependent launch of the next one)
@@ -860,7 +885,7 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
     // input block [offsets | x | y | z], 16-byte aligned parts, packed in pinned memory: ONE host-to-device copy
     const InBlock ib = in_block(ctx, n_hits_total);
     const FillPlan &pl1 = plan_fill(ctx, 1, n_hits_total, true);
-    const bool zero_copy = n_events == 1 && !ctx->tun.host_copy_input && pl1.ok && pl1.mode == 1;
+    const bool zero_copy = n_events == 1 && ctx->tun.host_copy_input != 1 && pl1.ok && pl1.mode == 1;
     const unsigned char *in_base = zero_copy ? sl.d_in_mapped : sl.d_in;
     if (n_hits_total > 0) {
         const size_t nb = sizeof(float) * (size_t)n_hits_total;
@@ -883,7 +908,7 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
         else
             HT_CUDA(cudaMemcpyAsync(sl.d_in, sl.h_in, sizeof(int32_t) * (size_t)(ne + 1), cudaMemcpyHostToDevice, st));
         const uint32_t room = capacity - written;
-        const int rc = enqueue_group(ctx, sl, in_base, ib, hb, ne, nh, ctx->d_hmh, threshold, room, false);
+        const int rc = enqueue_group(ctx, sl, in_base, ib, hb, ne, nh, ctx->d_hmh, threshold, room, kInputsPlain);
         if (rc != HT_OK) return rc;
         if (h_mh_or_null)
             HT_CUDA(cudaMemcpyAsync(h_mh_or_null + (size_t)e0 * cells, ctx->d_hmh, sizeof(uint32_t) * cells * (size_t)ne,

@@ -402,7 +402,7 @@ def test_submit_wait_host_pipeline():
     bn = Binning(4, 16, 256, 256)
     events = [generate_batch(wl, n_events=1, first_event=e) for e in range(7)]
     wants = [oracle_peaks(bn, oracle_fill(bn, *b.event(0))[0], wl.threshold) for b in events]
-    for tuning in (None, {"host_copy_input": 1}):
+    for tuning in (None, {"host_copy_input": 1}, {"host_copy_input": 2}):
         with GpuHough(bn, 1, 6000, host_slots=3, host_peak_capacity=4096, tuning=tuning) as g:
             out = np.zeros(4096, B.PEAK_DTYPE)
             in_flight = {}
@@ -567,7 +567,7 @@ def test_division_shortcut_equals_fdiv_rn_on_four_billion_pairs():
     assert B.ht_selftest_division(0, 100_000_000, 987654321) == 0
 
 
-@pytest.mark.parametrize("copy_input", [0, 1])
+@pytest.mark.parametrize("copy_input", [0, 1, 2])
 def test_run_host_single_event_zero_copy_and_copy(copy_input):
     """One event through ht_run_host: the kernel reads the hits straight from the pinned block (default) or the block is
     copied to the device first; same matrix, same peaks, several calls in a row on one context."""
@@ -601,7 +601,7 @@ def test_run_host_events_pipelines_a_sequence():
     batch = batch_from_arrays(evs)
     wants = [oracle_peaks(bn, oracle_fill(bn, *batch.event(e))[0], wl.threshold) for e in range(batch.n_events)]
     assert max(len(w) for w in wants) > 20 and len(wants[3]) == 0
-    for slots, tuning in ((1, None), (2, {"host_copy_input": 1}), (3, None)):
+    for slots, tuning in ((1, None), (2, {"host_copy_input": 1}), (3, {"host_copy_input": 2}), (3, {"fill_early_cap": -1})):
         with GpuHough(bn, 1, 4000, host_slots=slots, host_peak_capacity=4096, tuning=tuning) as g:
             for cap_ev in (4096, 16):
                 out = np.zeros(batch.n_events * cap_ev, B.PEAK_DTYPE)
@@ -624,6 +624,39 @@ def test_run_host_events_pipelines_a_sequence():
             with pytest.raises(B.HtError):
                 big = batch_from_arrays([np.ones((4001, 3), np.float32)])
                 B.ht_run_host_events(g.ctx, big.x, big.y, big.z, big.event_offsets, 1, wl.threshold, out, 16, nf)
+
+
+@pytest.mark.parametrize("copy_input", [1, 2])
+def test_host_pipeline_three_thousand_events(copy_input):
+    """The host path's hand-rolled synchronisation under load: the kernel waits for a word the copy stream writes behind
+    the hits, writes its peak records straight into pinned host memory, and ONE system-wide fence (the last CTA's) stands
+    between the records of all CTAs and the completion word the host polls.  3000 events through 4 slots; twelve distinct
+    events in turn, so that a slot never holds the same event twice running and a stale record or count cannot pass."""
+    bn = Binning(4, 16, 128, 128)
+    thr = 4
+    evs = []
+    for e in range(12):
+        b = generate_batch(WORKLOADS[3], n_events=1, first_event=e)
+        evs.append(np.stack(b.event(0), -1)[: 1500 + 100 * e])
+    wants = []
+    for ev in evs:
+        one = batch_from_arrays([ev])
+        wants.append(oracle_peaks(bn, oracle_fill(bn, *one.event(0))[0], thr))
+    assert min(len(w) for w in wants) > 50 and len({len(w) for w in wants}) > 6
+    n_rep = 250
+    batch = batch_from_arrays(evs * n_rep)
+    cap_ev = max(len(w) for w in wants)
+    with GpuHough(bn, 1, 3000, host_slots=4, host_peak_capacity=cap_ev, tuning={"host_copy_input": copy_input}) as g:
+        out = np.zeros(batch.n_events * cap_ev, B.PEAK_DTYPE)
+        nf = np.zeros(batch.n_events, np.uint32)
+        B.ht_run_host_events(g.ctx, batch.x, batch.y, batch.z, batch.event_offsets, batch.n_events, thr, out, cap_ev, nf)
+    for e in range(batch.n_events):
+        want = wants[e % 12]
+        assert nf[e] == len(want), e
+        got = out[e * cap_ev: e * cap_ev + len(want)]
+        got = got[np.argsort(got["cell"])]
+        assert np.all(got["event"] == e)
+        assert np.array_equal(got["cell"], want["cell"]) and np.array_equal(got["count"], want["count"]), e
 
 
 # ------------------------------------------------------------------ f3: track read-out of the peaks
