@@ -118,7 +118,12 @@ typedef struct ht_tuning {
     int32_t fill_early_cap;            /* single events of <= 32768 hits: every CTA finds the hits of its first tile's plane
                                           itself and votes while the grid still classifies ("early tiles").  > 0: records of
                                           that list in shared memory; 0: three times the average plane + 32; -1: no early tiles */
-    int32_t reserved[7];               /* must be zero */
+    int32_t host_direct_results;       /* single host events: 1: the kernel stores count and peak list straight into the pinned
+                                          result block (a kernel that does cannot complete before PCIe has acknowledged the
+                                          stores: +3.3 us per call); 0: into device memory, from where a copy stream that waits
+                                          for the kernel's completion word (cuStreamWaitValue32) brings them to the host -- or
+                                          as 1 where the driver has no such operation */
+    int32_t reserved[6];               /* must be zero */
 } ht_tuning;
 
 /* Sizes implied by a configuration: bytes of one event's matrix, and bytes of the context's device workspace

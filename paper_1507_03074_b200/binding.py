@@ -64,7 +64,8 @@ class ht_tuning(C.Structure):
     _fields_ = [("fill_batch_classification", C.c_int32), ("fill_slab_kb", C.c_int32),
                 ("fill_plain_stores", C.c_int32), ("cooperative_launch", C.c_int32),
                 ("host_copy_input", C.c_int32), ("peaks_unroll", C.c_int32), ("peaks_ctas_per_sm", C.c_int32),
-                ("fill_store_warps", C.c_int32), ("fill_early_cap", C.c_int32), ("reserved", C.c_int32 * 7)]
+                ("fill_store_warps", C.c_int32), ("fill_early_cap", C.c_int32), ("host_direct_results", C.c_int32),
+                ("reserved", C.c_int32 * 6)]
 
 
 class HtError(RuntimeError):

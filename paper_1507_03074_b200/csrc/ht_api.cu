@@ -7,6 +7,8 @@
 #include "ht_diag.cuh"
 #include "ht_merge.cuh"
 
+#include <cuda.h>      // types of the one driver entry point used (cuStreamWaitValue32, fetched through cudaGetDriverEntryPoint: no link to libcuda)
+
 #include <algorithm>
 #include <atomic>
 #include <cmath>
@@ -120,6 +122,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 constexpr size_t kBucketBytesMax = 32u << 20;   // cap of the single-event bucket region (bigger events take the batch path)
 constexpr size_t kZeroBytes = 232448;           // 227 KB: no slab is larger
+constexpr uint32_t kHostEagerPeaks = 4096;   // results through the copy engine: records copied to the host unasked (more: fetched by ht_wait_host)
 constexpr size_t kResHeader = 16;      // result block: [uint32 n_found, pad to 16][ht_peak x host_peak_capacity]
 
 // Layout of the context's device workspace (one contiguous block: caller-owned or allocated by ht_create) and sizes of
@@ -127,7 +130,7 @@ constexpr size_t kResHeader = 16;      // result block: [uint32 n_found, pad to 
 constexpr size_t kInTrailer = 16;     // last bytes of a slot's input block: the number of the submission whose hits the block holds
 
 struct WorkspaceLayout {
-    size_t tables, counters, hits, buckets, bucket_start, counts, counts1, zeros, in_dev, mh;      // offsets
+    size_t tables, counters, hits, buckets, bucket_start, counts, counts1, zeros, in_dev, res_dev, mh;      // offsets
     size_t hits_part;             // bytes of one of the 6 per-hit arrays
     size_t buckets_bytes;         // single-event classification: P buckets of n_hits records each (as far as this holds them)
     size_t in_block, res_block;   // bytes of ONE slot's input block [offsets | x | y | z] and result block
@@ -156,6 +159,7 @@ WorkspaceLayout workspace_layout(const ht_config *c)
                               3 * align_up(sizeof(float) * (size_t)c->max_hits, 16) + kInTrailer, 256);
         w.res_block = align_up(kResHeader + sizeof(ht_peak) * (size_t)c->host_peak_capacity, 256);
         w.in_dev = take(w.in_block * (size_t)c->host_slots);
+        w.res_dev = take(w.res_block * (size_t)c->host_slots);
         w.mh = take(cells * sizeof(uint32_t) * (size_t)c->host_slots);
     }
     w.total = off;
@@ -175,6 +179,8 @@ struct FillPlan {
 struct HostSlot {
     unsigned char *h_in = nullptr, *d_in = nullptr, *d_in_mapped = nullptr;   // pinned input block, its device mirror, its device alias
     unsigned char *h_res = nullptr, *d_res = nullptr;                          // mapped pinned result block and its device alias
+    unsigned char *d_res_dev = nullptr;                                        // result block in device memory (results through the copy engine)
+    bool via_copy = false;             // this submission's results: kernel -> d_res_dev -> (copy engine) -> h_res
     cudaEvent_t copied = nullptr, done = nullptr;
     bool busy = false;
     uint32_t seq = 0;                  // number of the slot's last submission (the kernel writes it into the result header)
@@ -220,7 +226,9 @@ struct ht_ctx {
     unsigned char *h_in_all = nullptr, *h_res_all = nullptr;
     std::vector<HostSlot> slots;
     uint32_t *d_hmh = nullptr;
-    cudaStream_t host_stream = nullptr, copy_stream = nullptr;
+    cudaStream_t host_stream = nullptr, copy_stream = nullptr, d2h_stream = nullptr;
+    // cuStreamWaitValue32 (nullptr: not available): lets the copy engine, not the kernel, carry a host event's results
+    CUresult (*stream_wait_value32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int) = nullptr;
     int64_t launches = 0;
     int32_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 };
@@ -392,13 +400,25 @@ int ht_create_ex(const ht_config *cfg, const ht_tuning *tuning, void *d_workspac
             sl.h_in = ctx->h_in_all + s * lay.in_block;
             sl.d_in_mapped = in_map + s * lay.in_block;
             sl.d_in = ws + lay.in_dev + s * lay.in_block;
+            sl.d_res_dev = ws + lay.res_dev + s * lay.res_block;
             sl.h_res = ctx->h_res_all + s * lay.res_block;
             sl.d_res = res_map + s * lay.res_block;
             if ((e = cudaEventCreateWithFlags(&sl.copied, cudaEventDisableTiming)) != cudaSuccess ||
                 (e = cudaEventCreateWithFlags(&sl.done, cudaEventDisableTiming)) != cudaSuccess)
                 return fail(cuda_fail(e, "cudaEventCreate(slot)"));
         }
+        if ((e = cudaMemset(ws + lay.res_dev, 0, lay.res_block * ns)) != cudaSuccess)
+            return fail(cuda_fail(e, "cudaMemset(result blocks)"));
+        if (!tun.host_direct_results) {
+            void *fn = nullptr;
+            cudaDriverEntryPointQueryResult qr = cudaDriverEntryPointSymbolNotFound;
+            if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &fn, cudaEnableDefault, &qr) == cudaSuccess &&
+                qr == cudaDriverEntryPointSuccess && fn != nullptr)
+                ctx->stream_wait_value32 = reinterpret_cast<CUresult (*)(CUstream, CUdeviceptr, cuuint32_t, unsigned int)>(fn);
+            (void)cudaGetLastError();
+        }
         if ((e = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking)) != cudaSuccess ||
+            (e = cudaStreamCreateWithFlags(&ctx->d2h_stream, cudaStreamNonBlocking)) != cudaSuccess ||
             (e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaStreamCreate"));
     }
@@ -524,7 +544,7 @@ enum { kInputsPlain = 0, kInputsStable = 1, kInputsHostMapped = 2 };
 int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_z, const int32_t *d_off, int32_t n_events,
                 int32_t n_hits_total, uint32_t *d_mh, bool peaks, uint32_t threshold, ht_peak *d_out, uint32_t capacity,
                 uint32_t *d_n_found, cudaStream_t st, int input_kind, uint32_t *d_done_flag = nullptr, uint32_t done_value = 0u,
-                const uint32_t *d_ready_flag = nullptr)
+                const uint32_t *d_ready_flag = nullptr, bool done_flag_on_device = false)
 {
     const bool early_inputs = input_kind != kInputsPlain;
     const ht::Geom &g = ctx->geom;
@@ -569,6 +589,7 @@ int launch_fill(ht_ctx *ctx, const float *d_x, const float *d_y, const float *d_
     a.done_flag = d_done_flag;
     a.done_value = done_value;
     a.ready_flag = d_ready_flag;        // (its value: done_value, the number of the submission)
+    a.done_flag_on_device = done_flag_on_device ? 1 : 0;
     a.threshold = threshold;
     static_assert(sizeof(ht::PeakOut) == sizeof(ht_peak), "peak record layout");
     a.out = reinterpret_cast<ht::PeakOut *>(d_out);
@@ -738,21 +759,27 @@ InBlock in_block(const ht_ctx *ctx, int32_t n_hits)
 // fused kernel (or the two-call path for shapes it refuses), peak list and count into slot s's mapped result block.
 int enqueue_group(ht_ctx *ctx, HostSlot &sl, const unsigned char *in_base, const InBlock &ib, int32_t hit_base, int32_t ne,
                   int32_t nh, uint32_t *d_mh, uint32_t threshold, uint32_t room, int input_kind, bool flag = false,
-                  const uint32_t *d_ready_flag = nullptr)
+                  const uint32_t *d_ready_flag = nullptr, bool results_in_device_memory = false)
 {
     cudaStream_t st = ctx->host_stream;
     const float *d_x = reinterpret_cast<const float *>(in_base + ib.o_x) + hit_base;
     const float *d_y = reinterpret_cast<const float *>(in_base + ib.o_y) + hit_base;
     const float *d_z = reinterpret_cast<const float *>(in_base + ib.o_z) + hit_base;
     const int32_t *d_off = reinterpret_cast<const int32_t *>(in_base);
-    uint32_t *d_count = reinterpret_cast<uint32_t *>(sl.d_res);
-    ht_peak *d_list = reinterpret_cast<ht_peak *>(sl.d_res + kResHeader);
-    // the kernel itself tells the host when the results are in the mapped block (second word of the header)
+    unsigned char *res = results_in_device_memory ? sl.d_res_dev : sl.d_res;
+    uint32_t *d_count = reinterpret_cast<uint32_t *>(res);
+    ht_peak *d_list = reinterpret_cast<ht_peak *>(res + kResHeader);
+    // the kernel itself says when the results are in the block (second word of the header): to the host, which polls the
+    // mapped block, or to the copy engine, which waits for the word in device memory and then copies the block
     sl.flagged = flag;
+    sl.via_copy = flag && results_in_device_memory;
     int rc = launch_fill(ctx, d_x, d_y, d_z, d_off, ne, nh, d_mh, true, threshold, d_list, room, d_count, st,
-                         input_kind, flag ? d_count + 1 : nullptr, sl.seq, d_ready_flag);
+                         input_kind, flag ? d_count + 1 : nullptr, sl.seq, d_ready_flag, results_in_device_memory);
     if (rc == HT_ERR_UNSUPPORTED) {
         sl.flagged = false;
+        sl.via_copy = false;
+        d_count = reinterpret_cast<uint32_t *>(sl.d_res);
+        d_list = reinterpret_cast<ht_peak *>(sl.d_res + kResHeader);
         if (d_ready_flag) {             // (the other kernels do not look at the copy's word: order the streams instead)
             HT_CUDA(cudaEventRecord(sl.copied, ctx->copy_stream));
             HT_CUDA(cudaStreamWaitEvent(st, sl.copied, 0));
@@ -813,12 +840,32 @@ int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y
     }
     // (the slot's blocks are the library's own: final before the kernel reads them -- host-mapped, or announced by the
     // copy stream)
+    const bool via_copy = ctx->stream_wait_value32 != nullptr;
     const int rc = enqueue_group(ctx, sl, in_base, ib, 0, 1, n_hits, d_mh, threshold, ctx->cfg.host_peak_capacity,
-                                 zero_copy ? kInputsHostMapped : kInputsStable, true, d_ready);
+                                 zero_copy ? kInputsHostMapped : kInputsStable, true, d_ready, via_copy);
     if (rc != HT_OK) return rc;
     // (no event between two kernels of the stream when the kernel signals its own completion: an event record there
     // would undo the dependent launch of the next one)
     if (!sl.flagged) HT_CUDA(cudaEventRecord(sl.done, ctx->host_stream));
+    if (sl.via_copy) {
+        // Results through the copy engine: the kernel writes count, list and -- last -- the submission's number into the
+        // slot's block in DEVICE memory; a third stream waits for that number (a stream memory operation: no event in the
+        // compute stream) and copies the head of the list, then the header, into the pinned block the host polls.  Peak
+        // records stored straight into pinned host memory keep a kernel from completing until PCIe has acknowledged them:
+        // 3.3 us per call that the next kernel of the stream has to wait for.
+        const uint32_t eager = std::min(ctx->cfg.host_peak_capacity, kHostEagerPeaks);
+        const CUresult wr = ctx->stream_wait_value32(reinterpret_cast<CUstream>(ctx->d2h_stream),
+                                                     reinterpret_cast<CUdeviceptr>(sl.d_res_dev + sizeof(uint32_t)), sl.seq,
+                                                     CU_STREAM_WAIT_VALUE_EQ);
+        if (wr != CUDA_SUCCESS) {
+            std::snprintf(g_cuda_err, sizeof g_cuda_err, "CUDA error in cuStreamWaitValue32: CUresult %d", (int)wr);
+            return HT_ERR_CUDA;
+        }
+        if (eager > 0)
+            HT_CUDA(cudaMemcpyAsync(sl.h_res + kResHeader, sl.d_res_dev + kResHeader, sizeof(ht_peak) * (size_t)eager,
+                                    cudaMemcpyDeviceToHost, ctx->d2h_stream));
+        HT_CUDA(cudaMemcpyAsync(sl.h_res, sl.d_res_dev, kResHeader, cudaMemcpyDeviceToHost, ctx->d2h_stream));
+    }
     sl.busy = true;
     return HT_OK;
 }
@@ -835,7 +882,7 @@ int ht_wait_host(ht_ctx *ctx, int32_t slot, ht_peak *h_out, uint32_t capacity, u
         const volatile uint32_t *flag = reinterpret_cast<const volatile uint32_t *>(sl.h_res) + 1;
         for (uint32_t spins = 0; *flag != sl.seq; ++spins) {
             if ((spins & 0xFFFu) == 0xFFFu) {                     // a failed kernel never writes the flag
-                const cudaError_t q = cudaStreamQuery(ctx->host_stream);
+                const cudaError_t q = cudaStreamQuery(sl.via_copy ? ctx->d2h_stream : ctx->host_stream);   // (whoever writes the word)
                 if (q != cudaSuccess && q != cudaErrorNotReady) return cuda_fail(q, "ht_wait_host");
                 if (q == cudaSuccess && *flag != sl.seq) return cuda_fail(cudaErrorUnknown, "ht_wait_host: stream idle, no result");
             }
@@ -848,7 +895,15 @@ int ht_wait_host(ht_ctx *ctx, int32_t slot, ht_peak *h_out, uint32_t capacity, u
     const uint32_t found = *reinterpret_cast<const volatile uint32_t *>(sl.h_res);
     uint32_t got = found < ctx->cfg.host_peak_capacity ? found : ctx->cfg.host_peak_capacity;
     if (got > capacity) got = capacity;
-    if (got > 0) std::memcpy(h_out, sl.h_res + kResHeader, sizeof(ht_peak) * (size_t)got);
+    if (sl.flagged && sl.via_copy && got > kHostEagerPeaks) {
+        // the list is longer than what the copy engine brought along: the rest straight from the slot's device block
+        // (the kernel has completed; a synchronous copy on the legacy stream, which the context's streams do not join)
+        std::memcpy(h_out, sl.h_res + kResHeader, sizeof(ht_peak) * (size_t)kHostEagerPeaks);
+        HT_CUDA(cudaMemcpy(h_out + kHostEagerPeaks, sl.d_res_dev + kResHeader + sizeof(ht_peak) * (size_t)kHostEagerPeaks,
+                           sizeof(ht_peak) * (size_t)(got - kHostEagerPeaks), cudaMemcpyDeviceToHost));
+    } else if (got > 0) {
+        std::memcpy(h_out, sl.h_res + kResHeader, sizeof(ht_peak) * (size_t)got);
+    }
     *h_n_found = found;
     return HT_OK;
 }
@@ -1154,6 +1209,7 @@ void ht_destroy(ht_ctx *ctx)
     DeviceGuard guard(ctx->cfg.device);
     if (ctx->host_stream) { cudaStreamSynchronize(ctx->host_stream); cudaStreamDestroy(ctx->host_stream); }
     if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
+    if (ctx->d2h_stream) { cudaStreamSynchronize(ctx->d2h_stream); cudaStreamDestroy(ctx->d2h_stream); }
     for (HostSlot &s : ctx->slots) {
         if (s.copied) cudaEventDestroy(s.copied);
         if (s.done) cudaEventDestroy(s.done);

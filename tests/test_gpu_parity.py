@@ -402,7 +402,7 @@ def test_submit_wait_host_pipeline():
     bn = Binning(4, 16, 256, 256)
     events = [generate_batch(wl, n_events=1, first_event=e) for e in range(7)]
     wants = [oracle_peaks(bn, oracle_fill(bn, *b.event(0))[0], wl.threshold) for b in events]
-    for tuning in (None, {"host_copy_input": 1}, {"host_copy_input": 2}):
+    for tuning in (None, {"host_copy_input": 1}, {"host_copy_input": 2}, {"host_direct_results": 1}):
         with GpuHough(bn, 1, 6000, host_slots=3, host_peak_capacity=4096, tuning=tuning) as g:
             out = np.zeros(4096, B.PEAK_DTYPE)
             in_flight = {}
@@ -601,7 +601,8 @@ def test_run_host_events_pipelines_a_sequence():
     batch = batch_from_arrays(evs)
     wants = [oracle_peaks(bn, oracle_fill(bn, *batch.event(e))[0], wl.threshold) for e in range(batch.n_events)]
     assert max(len(w) for w in wants) > 20 and len(wants[3]) == 0
-    for slots, tuning in ((1, None), (2, {"host_copy_input": 1}), (3, {"host_copy_input": 2}), (3, {"fill_early_cap": -1})):
+    for slots, tuning in ((1, None), (2, {"host_copy_input": 1}), (3, {"host_copy_input": 2}), (3, {"fill_early_cap": -1}),
+                          (2, {"host_direct_results": 1})):
         with GpuHough(bn, 1, 4000, host_slots=slots, host_peak_capacity=4096, tuning=tuning) as g:
             for cap_ev in (4096, 16):
                 out = np.zeros(batch.n_events * cap_ev, B.PEAK_DTYPE)
@@ -626,11 +627,12 @@ def test_run_host_events_pipelines_a_sequence():
                 B.ht_run_host_events(g.ctx, big.x, big.y, big.z, big.event_offsets, 1, wl.threshold, out, 16, nf)
 
 
-@pytest.mark.parametrize("copy_input", [1, 2])
-def test_host_pipeline_three_thousand_events(copy_input):
+@pytest.mark.parametrize("copy_input,direct", [(1, 0), (2, 0), (1, 1)])
+def test_host_pipeline_three_thousand_events(copy_input, direct):
     """The host path's hand-rolled synchronisation under load: the kernel waits for a word the copy stream writes behind
-    the hits, writes its peak records straight into pinned host memory, and ONE system-wide fence (the last CTA's) stands
-    between the records of all CTAs and the completion word the host polls.  3000 events through 4 slots; twelve distinct
+    the hits; its results reach the host through a copy stream that waits for the kernel's completion word, or (direct)
+    the kernel writes them straight into pinned host memory, where ONE system-wide fence (the last CTA's) stands between
+    the records of all CTAs and the completion word the host polls.  3000 events through 4 slots; twelve distinct
     events in turn, so that a slot never holds the same event twice running and a stale record or count cannot pass."""
     bn = Binning(4, 16, 128, 128)
     thr = 4
@@ -646,7 +648,8 @@ def test_host_pipeline_three_thousand_events(copy_input):
     n_rep = 250
     batch = batch_from_arrays(evs * n_rep)
     cap_ev = max(len(w) for w in wants)
-    with GpuHough(bn, 1, 3000, host_slots=4, host_peak_capacity=cap_ev, tuning={"host_copy_input": copy_input}) as g:
+    with GpuHough(bn, 1, 3000, host_slots=4, host_peak_capacity=cap_ev,
+                  tuning={"host_copy_input": copy_input, "host_direct_results": direct}) as g:
         out = np.zeros(batch.n_events * cap_ev, B.PEAK_DTYPE)
         nf = np.zeros(batch.n_events, np.uint32)
         B.ht_run_host_events(g.ctx, batch.x, batch.y, batch.z, batch.event_offsets, batch.n_events, thr, out, cap_ev, nf)
