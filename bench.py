@@ -12,7 +12,7 @@ value     events/s with the hits already resident in HBM: W warm-up steps, then 
           `--reps` (5) such brackets of plain stream launches (fixed rule, stated in config.launch_mode; the same calls
           replayed from a CUDA graph and the two-kernel split are reported beside it, each with its own median).
 e2e       the same metric through the C ABI with HOST buffers: ht_submit_host / ht_wait_host over the context's pinned
-          slots (hits cross PCIe inside the timed region, the kernel writes the peak list into mapped pinned memory).
+          slots (hits cross PCIe inside the timed region, count and peak list come back the same way).
 roofline  achieved = algorithmic bytes of one call (the matrix once + hits + peaks) / the call's average
           duration in the timed region; peak = MEASURED_PEAKS.json; store ceilings (cudaMemsetAsync of the same output
           matrices) measured in the same run; traffic from profiles/r02_traffic.json (an ncu capture) when it matches.
@@ -456,8 +456,11 @@ def bench_ours(args):
         B.ht_run_host(ctx, hx, hy, hz, hoff_t, n_ev, n_hits, T, houts[0], cap)
     e2e_sync_ms = max_over_ranks((time.perf_counter() - t0) * 1e3) / K
     e2e_value = jobs * n_ev * 1e3 / e2e_ms
-    h2d = 3 * 4 * n_hits                                   # x, y, z of the step's events (read by the kernel from the pinned block)
-    d2h = n_ev * 4 + 12 * min(n_found, cap * n_ev)         # counts + peak records, written by the kernel into mapped pinned memory
+    # per event: the packed input block [2 offsets | x | y | z] + the submission's number, copied to the device on the copy
+    # stream (or, for events too large for early tiles, read by the kernel from the pinned block: the same hit bytes); back:
+    # the result header + the head of the peak list (at most 4096 records, whatever the list holds), by the copy engine
+    h2d = 3 * 4 * n_hits + n_ev * (8 + 4)
+    d2h = n_ev * (16 + 12 * min(cap, 4096))
 
     # ---- N > 1: merge the ranks' peak lists over NCCL ("eventually the results are merged"), outside the timed region
     k_out = min(n_found, cap)
@@ -607,8 +610,10 @@ def bench_ours(args):
                     "ms_per_step": e2e_ms, "brackets": spread(e2e_reps), "slots": host_slots,
                     "sync_ms_per_step": e2e_sync_ms, "sync_events_per_s": jobs * n_ev * 1e3 / e2e_sync_ms,
                     "api": "ht_run_host_events: K steps' events as one sequence in host memory, one fused kernel per event, pipelined "
-                           "by the library over its pinned slots (ht_submit_host / ht_wait_host: the kernel reads the hits over "
-                           "PCIe, zero-copy, and writes the peak list into mapped pinned memory; up to `slots` events in flight); "
+                           "by the library over its pinned slots (ht_submit_host / ht_wait_host: an asynchronous copy brings the "
+                           "hits to the device and announces itself with a word the kernel waits for; count and peak list come back "
+                           "through a copy stream that waits for the kernel's completion word; no event between two kernels, up to "
+                           "`slots` events in flight); "
                            "sync_*: ht_run_host, one step at a time"},
             "tracking": tracking,
             "gpu_launches": int(launches_per_step * K),

@@ -274,7 +274,8 @@ HT_API int ht_match_truth(ht_ctx *ctx, const ht_candidate *d_cand, uint32_t n_ca
  * Packs offsets and hits into one pinned block, which the kernel reads directly (one event: every hit is read exactly
  * once, zero-copy over PCIe) or which is copied to the device in one transfer (batches, ht_tuning.host_copy_input),
  * runs ht_fill_peaks (or ht_fill + ht_peaks where that is unsupported) on the context's own matrices (events in groups
- * of host_slots) with the peak list and count written by the kernel straight into mapped pinned memory, and
+ * of host_slots) with the peak list and count written by the kernel straight into mapped pinned memory (the route with
+ * the fewest operations between the host's hits and the host's result: nothing else is in flight to overlap with), and
  * synchronises.  h_out receives min(*h_n_found, capacity) records; capacity <= cfg.host_peak_capacity.
  * h_mh_or_null: if not NULL, n_events * cells uint32 that also receive the matrices (testing; slow).
  * Host buffers may be pageable or pinned.  No event may be in flight in a slot (ht_submit_host without ht_wait_host).
@@ -290,11 +291,15 @@ HT_API int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const fl
  *                   (0 <= slot < cfg.host_slots; the caller's arrays may be reused as soon as the call returns),
  *                   enqueues the fused kernel (a0-a5; the event's matrix is materialised in the slot's own matrix) on the
  *                   context's stream and returns without waiting.  HT_ERR_INVALID_ARG if the slot still holds an event
- *                   that has not been waited for.  Events run in submission order.
+ *                   that has not been waited for.  Events run in submission order.  Between two events' kernels there is
+ *                   nothing in that stream (consecutive kernels keep their dependent launch): the hits reach the device
+ *                   through a copy stream whose last write is a word the kernel waits for (or are read by the kernel from
+ *                   the pinned block: ht_tuning.host_copy_input), count and peak list come back through a copy stream
+ *                   that waits for the kernel's completion word (ht_tuning.host_direct_results).
  *   ht_wait_host    blocks until the event submitted into `slot` has finished; h_out receives
  *                   min(*h_n_found, capacity, cfg.host_peak_capacity) records, *h_n_found the number of peaks found.
  *                   HT_ERR_INVALID_ARG if nothing was submitted into the slot.
- * ht_run_host on one event is ht_submit_host + ht_wait_host on slot 0.
+ * ht_run_host on one event is ht_submit_host + ht_wait_host on slot 0 (on the lone-event route described there).
  */
 HT_API int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y, const float *h_z, int32_t n_hits,
                           uint32_t threshold);

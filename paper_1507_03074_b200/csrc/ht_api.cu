@@ -796,8 +796,15 @@ int enqueue_group(ht_ctx *ctx, HostSlot &sl, const unsigned char *in_base, const
 
 extern "C" {
 
-int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y, const float *h_z, int32_t n_hits,
-                   uint32_t threshold)
+}  // extern "C"
+
+namespace {
+
+// ht_submit_host.  lone: the caller waits for this very event next (ht_run_host) -- nothing to overlap with, so the route
+// with the fewest operations between the host's hits and the host's result is taken (the kernel reads the hits from the
+// pinned block and stores its results into the pinned block), unless the tuning says otherwise.
+int submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y, const float *h_z, int32_t n_hits,
+                uint32_t threshold, bool lone)
 {
     if (!ctx) return HT_ERR_INVALID_ARG;
     if (ctx->cfg.host_slots < 1) return HT_ERR_UNSUPPORTED;
@@ -820,7 +827,7 @@ int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y
     // otherwise one packed copy on the copy stream, which overlaps the kernel of the previous event.
     const FillPlan &pl = plan_fill(ctx, 1, n_hits, true);
     // (early tiles -- every CTA reads all the hits -- want them in device memory: copy when the plan has them)
-    const bool want_copy = ctx->tun.host_copy_input == 1 || (ctx->tun.host_copy_input == 0 && pl.early_cap > 0);
+    const bool want_copy = ctx->tun.host_copy_input == 1 || (ctx->tun.host_copy_input == 0 && pl.early_cap > 0 && !lone);
     const bool zero_copy = !want_copy && pl.ok && pl.mode == 1;
     const unsigned char *in_base = sl.d_in_mapped;
     uint32_t *d_mh = ctx->d_hmh + (size_t)slot * (size_t)ctx->geom.cells;
@@ -840,7 +847,7 @@ int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y
     }
     // (the slot's blocks are the library's own: final before the kernel reads them -- host-mapped, or announced by the
     // copy stream)
-    const bool via_copy = ctx->stream_wait_value32 != nullptr;
+    const bool via_copy = ctx->stream_wait_value32 != nullptr && !lone;
     const int rc = enqueue_group(ctx, sl, in_base, ib, 0, 1, n_hits, d_mh, threshold, ctx->cfg.host_peak_capacity,
                                  zero_copy ? kInputsHostMapped : kInputsStable, true, d_ready, via_copy);
     if (rc != HT_OK) return rc;
@@ -868,6 +875,16 @@ int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y
     }
     sl.busy = true;
     return HT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ht_submit_host(ht_ctx *ctx, int32_t slot, const float *h_x, const float *h_y, const float *h_z, int32_t n_hits,
+                   uint32_t threshold)
+{
+    return submit_host(ctx, slot, h_x, h_y, h_z, n_hits, threshold, false);
 }
 
 int ht_wait_host(ht_ctx *ctx, int32_t slot, ht_peak *h_out, uint32_t capacity, uint32_t *h_n_found)
@@ -928,7 +945,7 @@ int ht_run_host(ht_ctx *ctx, const float *h_x, const float *h_y, const float *h_
 
     // one event without a matrix read-back: the asynchronous pair, back to back
     if (n_events == 1 && !h_mh_or_null) {
-        int rc = ht_submit_host(ctx, 0, h_x, h_y, h_z, n_hits_total, threshold);
+        int rc = submit_host(ctx, 0, h_x, h_y, h_z, n_hits_total, threshold, true);
         if (rc != HT_OK) return rc;
         return ht_wait_host(ctx, 0, h_out, capacity, h_n_found);
     }
