@@ -62,7 +62,8 @@ typedef enum ht_status {
                                 n_hits_total > max_hits, threshold == 0, cells >= 2^32 */
     HT_ERR_UNSUPPORTED = -2, /* binning does not fit the kernel (see ht_fill, ht_fill_peaks), or call unavailable */
     HT_ERR_CUDA = -3,        /* a CUDA runtime call or a launch failed */
-    HT_ERR_NOMEM = -4        /* host or device allocation failed */
+    HT_ERR_NOMEM = -4,       /* host or device allocation failed */
+    HT_ERR_TOO_LARGE = -5    /* a size beyond the fixed capacity of an entry point with static scratch (ht_merge_ridges_static) */
 } ht_status;
 
 typedef struct ht_ctx ht_ctx; /* opaque; created by ht_create, freed by ht_destroy */
@@ -242,6 +243,22 @@ typedef struct ht_candidate {
 HT_API size_t ht_merge_scratch_bytes(uint32_t n_peaks);
 HT_API int ht_merge_ridges(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, uint32_t window, ht_candidate *d_out,
                            uint32_t capacity, uint32_t *d_n_out, void *d_scratch, size_t scratch_bytes, void *cuda_stream);
+
+/*
+ * ht_merge_ridges for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments, same result, but the scratch is a file-scope device array of the
+ * library -- 3 * 4 * HT_MERGE_STATIC_MAX_PEAKS bytes = 768 KB, held by every GPU that loads the library until the process
+ * exits.  The call allocates nothing, on the device or through any library routine; the array's device address is looked
+ * up (cudaGetSymbolAddress) on the first call per device, so make that first call outside a graph capture.
+ *   n_peaks > HT_MERGE_STATIC_MAX_PEAKS: HT_ERR_TOO_LARGE, nothing is enqueued (use ht_merge_ridges).
+ * ALL calls on a device, from every context and thread, share the one array: two calls that overlap on the GPU (different
+ * streams without an ordering between them) race and give wrong candidates; calls of one stream, or stream-ordered like
+ * the other calls of a context, are safe.  The array keeps the last call's contents; nothing in it needs to start at zero
+ * (every word a call reads it has written itself), so no clearing happens between calls.
+ */
+#define HT_MERGE_STATIC_MAX_PEAKS 65536u
+HT_API int ht_merge_ridges_static(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, uint32_t window, ht_candidate *d_out,
+                                  uint32_t capacity, uint32_t *d_n_out, void *cuda_stream);
 
 /* A generated track for ht_match_truth: the centre (a, b) [mm] of its circle through the origin, R (q sin phi0, -q cos phi0). */
 typedef struct ht_truth {

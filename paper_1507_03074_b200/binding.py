@@ -14,7 +14,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libht.so")
 
-HT_OK, HT_ERR_INVALID_ARG, HT_ERR_UNSUPPORTED, HT_ERR_CUDA, HT_ERR_NOMEM = 0, -1, -2, -3, -4
+HT_OK, HT_ERR_INVALID_ARG, HT_ERR_UNSUPPORTED, HT_ERR_CUDA, HT_ERR_NOMEM, HT_ERR_TOO_LARGE = 0, -1, -2, -3, -4, -5
+HT_MERGE_STATIC_MAX_PEAKS = 65536
 
 PEAK_DTYPE = np.dtype([("event", np.uint32), ("cell", np.uint32), ("count", np.uint32)])   # == struct ht_peak
 
@@ -29,7 +30,7 @@ SUMMARY_DTYPE = np.dtype([("n_cand", np.int64), ("n_truth", np.int64), ("n_match
                           ("sum_drho2", np.float64), ("sum_dphi", np.float64), ("sum_dphi2", np.float64)])   # == ht_match_summary
 
 EXPORTS = ("ht_query_sizes", "ht_create", "ht_create_ex", "ht_fill", "ht_fill_peaks", "ht_promise_stable_inputs", "ht_fill_naive", "ht_peaks", "ht_tracks",
-           "ht_merge_scratch_bytes", "ht_merge_ridges", "ht_match_truth",
+           "ht_merge_scratch_bytes", "ht_merge_ridges", "ht_merge_ridges_static", "ht_match_truth",
            "ht_run_host", "ht_run_host_events", "ht_submit_host", "ht_wait_host", "ht_destroy", "ht_strerror")                  # include/ht.h
 DIAG_EXPORTS = ("ht_tables_host", "ht_kernel_launches", "ht_launch_info", "ht_selftest_division", "ht_diag_memset",
                 "ht_diag_vote_rates")                                                                     # include/ht_diag.h
@@ -120,6 +121,8 @@ def load() -> C.CDLL:
     lib.ht_merge_scratch_bytes.argtypes = [u32]
     lib.ht_merge_ridges.restype = C.c_int
     lib.ht_merge_ridges.argtypes = [vp, vp, u32, u32, vp, u32, vp, vp, C.c_size_t, vp]
+    lib.ht_merge_ridges_static.restype = C.c_int
+    lib.ht_merge_ridges_static.argtypes = [vp, vp, u32, u32, vp, u32, vp, vp]
     lib.ht_match_truth.restype = C.c_int
     lib.ht_match_truth.argtypes = [vp, vp, u32, vp, u32, C.c_double, C.c_double, vp, vp, vp, vp]
     lib.ht_run_host.restype = C.c_int
@@ -243,6 +246,12 @@ def ht_merge_ridges(ctx, d_peaks, n_peaks: int, window: int, d_out, capacity: in
     """Ridge merging of n_peaks peak records into track candidates (ht_candidate records, 6 words each)."""
     _check(load().ht_merge_ridges(ctx, _ptr(d_peaks), n_peaks, window, _ptr(d_out), capacity, _ptr(d_n_out), _ptr(d_scratch),
                                   scratch_bytes, _stream(stream)), "ht_merge_ridges")
+
+
+def ht_merge_ridges_static(ctx, d_peaks, n_peaks: int, window: int, d_out, capacity: int, d_n_out, stream=None) -> None:
+    """ht_merge_ridges on the library's static device scratch (at most HT_MERGE_STATIC_MAX_PEAKS peaks; allocates nothing)."""
+    _check(load().ht_merge_ridges_static(ctx, _ptr(d_peaks), n_peaks, window, _ptr(d_out), capacity, _ptr(d_n_out),
+                                         _stream(stream)), "ht_merge_ridges_static")
 
 
 def ht_match_truth(ctx, d_cand, n_cand: int, d_truth, n_truth: int, w_rho: float, cos_w_phi: float, d_cand_match,

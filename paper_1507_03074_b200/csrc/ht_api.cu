@@ -15,6 +15,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1091,6 +1092,57 @@ int ht_merge_ridges(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, uint3
     return HT_OK;
 }
 
+}  // extern "C"
+
+namespace {
+
+// Scratch of ht_merge_ridges_static: a file-scope device array (every GPU that loads the library holds these 768 KB until
+// the process exits).  In HOST code the name g_merge_scratch is a host-side stand-in, not a device address: the address a
+// kernel can use comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) uint32_t g_merge_scratch[3u * HT_MERGE_STATIC_MAX_PEAKS];
+
+constexpr int kMaxDevices = 64;
+std::mutex g_merge_scratch_mu;
+uint32_t *g_merge_scratch_addr[kMaxDevices] = {};
+
+// device address of g_merge_scratch on `device` (which must be current); looked up on the first call per device
+int merge_scratch_of_device(int device, uint32_t **out)
+{
+    if (device < 0 || device >= kMaxDevices) return HT_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_merge_scratch_mu);
+    if (!g_merge_scratch_addr[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_merge_scratch);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_merge_scratch)");
+        if (!p) return cuda_fail(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_merge_scratch): null address");
+        g_merge_scratch_addr[device] = static_cast<uint32_t *>(p);
+    }
+    *out = g_merge_scratch_addr[device];
+    return HT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ht_merge_ridges_static(ht_ctx *ctx, const ht_peak *d_peaks, uint32_t n_peaks, uint32_t window, ht_candidate *d_out,
+                           uint32_t capacity, uint32_t *d_n_out, void *cuda_stream)
+{
+    if (!ctx) return HT_ERR_INVALID_ARG;
+    if (n_peaks > HT_MERGE_STATIC_MAX_PEAKS) return HT_ERR_TOO_LARGE;     // (ht_strerror says what to call instead)
+    uint32_t *scratch = nullptr;
+    {
+        DeviceGuard guard(ctx->cfg.device);
+        if (guard.err != cudaSuccess) return cuda_fail(guard.err, "cudaSetDevice");
+        const int rc = merge_scratch_of_device(ctx->cfg.device, &scratch);
+        if (rc != HT_OK) return rc;
+    }
+    // the existing path, on the static array: every word of the scratch it reads it has written in the same call (slot per
+    // peak, order per kept peak, label per group member), so nothing needs clearing between calls
+    return ht_merge_ridges(ctx, d_peaks, n_peaks, window, d_out, capacity, d_n_out, scratch,
+                           sizeof(uint32_t) * 3u * (size_t)HT_MERGE_STATIC_MAX_PEAKS, cuda_stream);
+}
+
 int ht_match_truth(ht_ctx *ctx, const ht_candidate *d_cand, uint32_t n_cand, const ht_truth *d_truth, uint32_t n_truth, double w_rho,
                    double cos_w_phi, int32_t *d_cand_match, int32_t *d_truth_match, ht_match_summary *d_summary, void *cuda_stream)
 {
@@ -1246,6 +1298,9 @@ const char *ht_strerror(int status)
     case HT_ERR_UNSUPPORTED: return "binning not supported by this kernel (see include/ht.h) or call unavailable";
     case HT_ERR_CUDA: return g_cuda_err;
     case HT_ERR_NOMEM: return "out of memory";
+    case HT_ERR_TOO_LARGE:
+        return "more peaks than the static scratch of ht_merge_ridges_static holds (HT_MERGE_STATIC_MAX_PEAKS = 65536): "
+               "use ht_merge_ridges with caller-owned scratch";
     default: return "unknown status";
     }
 }
