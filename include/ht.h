@@ -17,7 +17,7 @@
  *     buffer it passes.  The context's device workspace (the angle tables, a few counters, the scratch of the
  *     classification: 24 bytes per hit of cfg.max_hits and 8 bytes per (event, plane) for batches, one bucket of 16-byte
  *     records per plane -- at most 32 MB -- and a 128-byte counter line per plane for single events, a 227 KB block of
- *     zeros; and, if cfg.host_slots > 0, the input mirror and host_slots vote matrices of the host calls) is either
+ *     zeros; and, if cfg.host_slots > 0, per slot an input mirror, a result block and a vote matrix of the host calls) is either
  *     handed in by the caller
  *     (ht_query_sizes -> allocate -> ht_create_ex: the library then allocates NOTHING on the device) or allocated by
  *     ht_create itself (convenience form).  With cfg.host_slots > 0 the context also owns pinned HOST staging blocks.

@@ -627,6 +627,45 @@ def test_run_host_events_pipelines_a_sequence():
                 B.ht_run_host_events(g.ctx, big.x, big.y, big.z, big.event_offsets, 1, wl.threshold, out, 16, nf)
 
 
+@pytest.mark.parametrize("direct", [0, 1])
+def test_host_event_with_more_peaks_than_the_copy_engine_brings_along(direct):
+    """Results through the copy engine: the copy stream brings the header and the first 4096 records to the host; a longer
+    list's tail is fetched from the slot's device block by ht_wait_host.  A dense event with well over 4096 peaks, read
+    back whole, then truncated at capacities on both sides of 4096; the direct route (the kernel stores into pinned
+    memory) must give the same lists."""
+    bn = Binning(4, 16, 256, 512)
+    thr = 10
+    batch = generate_batch(WORKLOADS[4], n_events=1)
+    want = oracle_peaks(bn, oracle_fill(bn, *batch.event(0))[0], thr)
+    assert 6000 < len(want) < 30000
+    cap = 1 << 15
+    with GpuHough(bn, 1, batch.n_hits, host_slots=2, host_peak_capacity=cap, tuning={"host_direct_results": direct}) as g:
+        for rep in range(2):                                          # (the second time the slot's blocks hold the first result)
+            out = np.zeros(cap, B.PEAK_DTYPE)
+            B.ht_submit_host(g.ctx, rep, batch.x, batch.y, batch.z, batch.n_hits, thr)
+            n = B.ht_wait_host(g.ctx, rep, out, cap)
+            assert n == len(want)
+            np.testing.assert_array_equal(sort_peaks(out[:n], bn.cells), want)
+        full = set(map(tuple, want.tolist()))
+        for part in (4095, 4096, 4097, 5000):
+            out = np.zeros(part, B.PEAK_DTYPE)
+            B.ht_submit_host(g.ctx, 0, batch.x, batch.y, batch.z, batch.n_hits, thr)
+            n = B.ht_wait_host(g.ctx, 0, out, part)
+            got = set(map(tuple, out.tolist()))
+            assert n == len(want) and len(got) == part and got <= full
+        # the pipelined form on the same event, twice in a row
+        out = np.zeros(2 * cap, B.PEAK_DTYPE)
+        nf = np.zeros(2, np.uint32)
+        two = batch_from_arrays([np.stack(batch.event(0), -1)] * 2)
+        B.ht_run_host_events(g.ctx, two.x, two.y, two.z, two.event_offsets, 2, thr, out, cap, nf)
+        for e in range(2):
+            assert nf[e] == len(want)
+            got = out[e * cap: e * cap + len(want)]
+            assert np.all(got["event"] == e)
+            got = got[np.argsort(got["cell"])]
+            assert np.array_equal(got["cell"], want["cell"]) and np.array_equal(got["count"], want["count"])
+
+
 @pytest.mark.parametrize("copy_input,direct", [(1, 0), (2, 0), (1, 1)])
 def test_host_pipeline_three_thousand_events(copy_input, direct):
     """The host path's hand-rolled synchronisation under load: the kernel waits for a word the copy stream writes behind
