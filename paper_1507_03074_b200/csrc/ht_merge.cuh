@@ -98,10 +98,11 @@ __global__ void merge_scatter_kernel(const PeakOut *__restrict__ peaks, uint32_t
 }
 
 // one CTA per (event, plane) group; order[] holds the peaks of group k at [start[k], start[k+1]); label[] is scratch.
-// Groups of up to kMergeSmem peaks keep their (a, b) cells and labels in shared memory (the pair loop reads them m times
-// per sweep); larger groups work on global memory.
-constexpr int kMergeThreads = 256;
+// Groups of up to kMergeSmem peaks keep their (a, b) cells, counts and labels in shared memory (sorted by cell when they
+// hold more than kMergeSortFrom peaks); larger groups work on global memory.
+constexpr int kMergeThreads = 1024;
 constexpr int kMergeSmem = 2048;
+constexpr int kMergeSortFrom = 192;  // groups with more peaks are sorted by cell first (config 2's planes hold ~12, at most ~70)
 
 __global__ void __launch_bounds__(kMergeThreads)
 merge_groups_kernel(const PeakOut *__restrict__ peaks, Geom g, const int32_t *__restrict__ start,
@@ -110,6 +111,7 @@ merge_groups_kernel(const PeakOut *__restrict__ peaks, Geom g, const int32_t *__
 {
     __shared__ uint32_t s_ab[kMergeSmem];                               // a << 16 | b  (both < 65536: checked by the host)
     __shared__ uint32_t s_label[kMergeSmem];
+    __shared__ uint32_t s_cnt[kMergeSmem];                              // the peaks' counts (the emission walks all members of a component)
     const int lo = start[blockIdx.x], hi = start[blockIdx.x + 1];
     const int m = hi - lo;
     if (m <= 0) return;
@@ -124,44 +126,119 @@ merge_groups_kernel(const PeakOut *__restrict__ peaks, Geom g, const int32_t *__
     for (int i = threadIdx.x; i < m; i += blockDim.x) {
         label[i] = (uint32_t)i;
         if (in_smem) {
-            const uint32_t cell = peaks[order[lo + i]].cell;
-            s_ab[i] = (((cell / NB) % NA) << 16) | (cell % NB);
+            const PeakOut p = peaks[order[lo + i]];
+            s_ab[i] = (((p.cell / NB) % NA) << 16) | (p.cell % NB);
+            s_cnt[i] = p.count;
         }
     }
     __syncthreads();
+    // A group in shared memory is sorted by cell (a, then b; bitonic, the counts travel along): the peaks that can be linked
+    // to position i -- |a - a_i| <= window -- are then a contiguous range around i, and a sweep tests a few dozen pairs per
+    // peak instead of m (a dense plane of a 20000-hit event holds a thousand peaks).  Positions, and with them roots,
+    // are positions of the sorted order; what is emitted does not depend on which member is the root.
+    const bool sorted = in_smem && m > kMergeSortFrom;                  // (small groups: the plain all-pairs sweep is faster)
+    if (sorted) {
+        int padded = 2;
+        while (padded < m) padded <<= 1;
+        for (int i = m + (int)threadIdx.x; i < padded; i += blockDim.x) {
+            s_ab[i] = 0xffffffffu;                                      // (above every key: a, b < 65536 and a < NA <= 65535)
+            s_cnt[i] = 0u;
+        }
+        __syncthreads();
+        for (int k = 2; k <= padded; k <<= 1) {
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                for (int i = threadIdx.x; i < padded; i += blockDim.x) {
+                    const int x = i ^ j;
+                    if (x > i) {
+                        const uint32_t ki = s_ab[i], kx = s_ab[x];
+                        const bool up = (i & k) == 0;
+                        if (up ? ki > kx : ki < kx) {
+                            s_ab[i] = kx;
+                            s_ab[x] = ki;
+                            const uint32_t c = s_cnt[i];
+                            s_cnt[i] = s_cnt[x];
+                            s_cnt[x] = c;
+                        }
+                    }
+                }
+                __syncthreads();
+            }
+        }
+    }
+    // Connected components by hooking and flattening.  A label is a position of the same component, never larger than the
+    // position that holds it; a position that holds itself is a root.  Every sweep starts with FLAT labels (each position
+    // holds its root): a position looks for the smallest root among the positions linked to it and hooks its OWN ROOT under
+    // it (atomicMin), which merges whole trees, not single positions -- a ridge of a thousand peaks converges in a handful
+    // of sweeps instead of one sweep per window length (20000-hit event, 1049 peaks in one plane: 3.9 ms -> see DESIGN.md);
+    // then every position follows its labels down to the root again.  No sweep hooks anything: every linked pair shares
+    // its root, and the root of a component is its smallest position, as before.
+    auto root_of = [&](uint32_t x) -> uint32_t {
+        for (uint32_t up = *reinterpret_cast<volatile uint32_t *>(&label[x]); up < x;
+             up = *reinterpret_cast<volatile uint32_t *>(&label[x])) x = up;
+        return x;
+    };
     for (;;) {
         int changed = 0;
         for (int i = threadIdx.x; i < m; i += blockDim.x) {
             const uint32_t abi = ab_of(i);
             const int ai = (int)(abi >> 16), bi = (int)(abi & 0xFFFFu);
-            uint32_t l = *reinterpret_cast<volatile uint32_t *>(&label[i]);
-            const uint32_t l0 = l;
-            for (int j = 0; j < m; ++j) {
+            uint32_t l = 0xffffffffu;
+            auto look = [&](int j) -> bool {                           // false: row a_j is more than `window` rows away
                 const uint32_t abj = ab_of(j);
                 const int da = abs(ai - (int)(abj >> 16)), db = abs(bi - (int)(abj & 0xFFFFu));
                 if ((uint32_t)max(da, db) <= window) l = min(l, *reinterpret_cast<volatile uint32_t *>(&label[j]));
+                return (uint32_t)da <= window;
+            };
+            if (sorted) {                                               // sorted by (a, b): outwards from i while the rows are near
+                for (int j = i; j >= 0 && look(j); --j) { }
+                for (int j = i + 1; j < m && look(j); ++j) { }
+            } else {
+                for (int j = 0; j < m; ++j) look(j);
             }
-            // follow the labels down to their current root (a label is a position of the same component, never larger
-            // than the position that holds it): long ridges converge in a few sweeps instead of one per link
-            for (uint32_t up = *reinterpret_cast<volatile uint32_t *>(&label[l]); up < l;
-                 up = *reinterpret_cast<volatile uint32_t *>(&label[l])) l = up;
-            if (l < l0) {
-                atomicMin(&label[i], l);
+            // (labels only ever decrease, and stay positions of the component: a label read while others hook is as good)
+            l = root_of(l);                                             // (i is linked to itself: l is a position)
+            const uint32_t mine = root_of((uint32_t)i);
+            if (l < mine) {
+                atomicMin(&label[mine], l);
                 changed = 1;
             }
         }
-        if (!__syncthreads_or(changed)) break;
+        const int any = __syncthreads_or(changed);
+        for (int i = threadIdx.x; i < m; i += blockDim.x) {
+            const uint32_t r = root_of((uint32_t)i);
+            if (r < (uint32_t)i) atomicMin(&label[i], r);
+        }
+        __syncthreads();
+        if (!any) break;
     }
     // roots (label == own position) emit their component
     for (int i = threadIdx.x; i < m; i += blockDim.x) {
         if (label[i] != (uint32_t)i) continue;
         uint32_t members = 0u;
         PeakOut best = peaks[order[lo + i]];
-        for (int j = 0; j < m; ++j) {
-            if (label[j] != (uint32_t)i) continue;
-            ++members;
-            const PeakOut p = peaks[order[lo + j]];
-            if (p.count > best.count || (p.count == best.count && p.cell < best.cell)) best = p;
+        if (in_smem) {
+            // all peaks of a group share event and plane: a member's cell follows from its (a, b).  (Position i of the
+            // sorted order is not peak order[lo + i]: the record above only lends its event and plane.)
+            const uint32_t plane_base = best.cell - (((best.cell / NB) % NA) * NB + best.cell % NB);
+            best.count = 0u;
+            best.cell = 0xffffffffu;
+            for (int j = 0; j < m; ++j) {
+                if (label[j] != (uint32_t)i) continue;
+                ++members;
+                const uint32_t abj = s_ab[j], cnt = s_cnt[j];
+                const uint32_t cell = plane_base + (abj >> 16) * NB + (abj & 0xFFFFu);
+                if (cnt > best.count || (cnt == best.count && cell < best.cell)) {
+                    best.count = cnt;
+                    best.cell = cell;
+                }
+            }
+        } else {
+            for (int j = 0; j < m; ++j) {
+                if (label[j] != (uint32_t)i) continue;
+                ++members;
+                const PeakOut p = peaks[order[lo + j]];
+                if (p.count > best.count || (p.count == best.count && p.cell < best.cell)) best = p;
+            }
         }
         const uint32_t at = atomicAdd(n_out, 1u);
         if (at < capacity) {

@@ -816,6 +816,34 @@ def test_ridge_merging_matches_the_oracle():
                 pk = np.concatenate([pk, pk[: n // 10]])            # duplicate records are linked at any window
             for w in (0, 1, 4):
                 _check_merge(g, bn, pk, w)
+    # large groups: more than 192 peaks of one plane are sorted by cell first (the sweeps then look at nearby rows only),
+    # more than 2048 work on global memory; long ridges, dense blobs, duplicates, every window from 0 to "everything"
+    bn = Binning(1, 2, 200, 300)
+    with GpuHough(bn, 2, 1) as g:
+        for trial, n in enumerate((700, 3000, 3900, 9000)):
+            keys = rng.choice(2 * bn.cells, size=n, replace=False)
+            pk = np.zeros(n, B.PEAK_DTYPE)
+            pk["event"], pk["cell"], pk["count"] = keys // bn.cells, keys % bn.cells, rng.integers(8, 11, n)
+            if trial % 2:
+                pk = np.concatenate([pk, pk[: n // 7]])
+            for w in (0, 1, 2, 5):
+                _check_merge(g, bn, pk, w)
+        # one diagonal ridge per plane (a chain of 190 links) plus noise: hooking has to carry a label along the whole chain
+        ridge = np.zeros(2 * 190 + 400, B.PEAK_DTYPE)
+        for p_ in range(2):
+            a = np.arange(190) + 5
+            ridge["cell"][p_ * 190:(p_ + 1) * 190] = (p_ * bn.n_a + a) * bn.n_b + (a + 20 + 3 * p_)
+        ridge["cell"][380:] = rng.choice(bn.cells, size=400, replace=False)
+        ridge["count"] = rng.integers(8, 40, len(ridge))
+        ridge = ridge[rng.permutation(len(ridge))]
+        for w in (1, 2, 3):
+            _check_merge(g, bn, ridge, w)
+    # the peaks of the 20000-hit event (about 200 per plane, a thousand in the densest)
+    wl = WORKLOADS[4]
+    with GpuHough(wl.binning, 1, 20000) as g:
+        _, n, pk = g.fill_peaks(generate_batch(wl, n_events=1), wl.threshold, store=False)
+        assert n == len(pk) > 10000
+        assert _check_merge(g, wl.binning, pk, 3) > _check_merge(g, wl.binning, pk, 10) > 500
 
 
 def test_truth_matching_matches_the_oracle():
