@@ -15,7 +15,7 @@ e2e       the same metric through the C ABI with HOST buffers: ht_submit_host / 
           slots (hits cross PCIe inside the timed region, count and peak list come back the same way).
 roofline  achieved = algorithmic bytes of one call (the matrix once + hits + peaks) / the call's average
           duration in the timed region; peak = MEASURED_PEAKS.json; store ceilings (cudaMemsetAsync of the same output
-          matrices) measured in the same run; traffic from profiles/r02_traffic.json (an ncu capture) when it matches.
+          matrices) measured in the same run; traffic from profiles/r02_traffic.csv (an ncu capture) when it matches.
 cpu_baseline  the CPU oracle as it stands on one core of this box (also the parity check of this very run), plus the
           same oracle on all cores, one event per process.
 N > 1 (torchrun): every rank its own events, no data-path collective ("weak"); `--split planes`: all ranks the same
@@ -476,10 +476,12 @@ def bench_ours(args):
 
         traffic, traffic_src = {}, None
         try:
-            with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as f:
-                tj = json.load(f)
-            if tj.get("workload") == f"config{wl.config}:{wl.name}" and tj.get("events_per_step") == n_ev and world == 1:
-                traffic, traffic_src = tj.get("dram_bytes_per_launch", {}), tj.get("source")
+            import csv
+            with open(os.path.join(ROOT, "profiles", "r02_traffic.csv"), newline="") as f:
+                for row in csv.DictReader(f):
+                    if row["workload"] == f"config{wl.config}:{wl.name}" and int(row["events_per_step"]) == n_ev and world == 1:
+                        traffic[row["entry_point"]] = float(row["dram_bytes_per_launch"])
+                        traffic_src = row["source"]
         except Exception:
             pass
 
